@@ -1,0 +1,120 @@
+"""Writes paper_2602_13198_b200/workloads_calibrated.json from short runs of the CPU ORACLE only.
+
+The five BASELINE.json configs leave three numbers per config open:
+  w_min    "minimum weight": f * max_k w(nu_k) of the weight table built with
+           w_min = 0; stored as w_min * N_s because Eq. 2 makes every weight proportional to 1/N_s.
+           f = 1e-6 for config 0 (sampled band 1e8-5e11 Hz); f = 1e-14 for config 1 (with 1e-6
+           the gate w/b >= w_min of the scattering test would suppress all but ~1 % of the events,
+           b reaching 25..625 there); f = 1e-17 for the torus
+           configs, whose weights span 1e49..1e27 between 1e8 and 1.6e11 Hz, so that the floor sits
+           1.5 decades above the nu L_nu peak and a child of weight w/b with b ~ 1e4-1e6 stays above
+           it (the paper's own floor, 1e28, is likewise ~1e-17 of its typical weights).
+  M_unit   mass unit of the torus configs.  BASELINE.json asks for ~2.5 Jy at 230 GHz; for this
+           synthetic torus (R_high = 40, beta = 100 => Theta_e ~ 0.4) the 230 GHz flux of the
+           oracle peaks near 0.5 Jy at M_unit ~ 1e23 (Thomson depth ~2) and collapses beyond it, so
+           the target is unreachable; M_unit = 5e19 is fixed instead, which gives the Thomson depths
+           BASELINE.json states for config 4 (tau_T ~ 1 after the x1e3 density scaling).  The
+           measured 230 GHz flux is stored for the record.
+  bias0    scattering bias amplitude (G21) tuned so that spawned / primaries ~ 7 for configs 2-3
+           ("7-10x"); config 1 uses 0.25/tau_T; config 4 is analog (b = 1).
+
+Run:  python oracle/calibrate.py        (about two minutes on 8 cores; deterministic)
+Nothing here touches the CUDA path.
+"""
+import json
+import math
+import os
+import sys
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+sys.path.insert(0, ROOT)
+sys.path.insert(0, os.path.join(ROOT, "tests"))
+
+from oracle_binding import Oracle  # noqa: E402
+from paper_2602_13198_b200 import workloads as wl  # noqa: E402
+
+OUT = os.path.join(ROOT, "paper_2602_13198_b200", "workloads_calibrated.json")
+M_UNIT_TORUS = 5e19
+SPAWN_TARGET = 7.0
+
+
+def wmin_per_ns(p, prim, f=1e-6):
+    q = dict(p)
+    q["w_min"] = 0.0
+    o = Oracle(q, prim)
+    o.prepare()
+    _, w = o.weight_table()
+    return f * float(w.max()) * q["Ns_target"]
+
+
+def tune_bias(p, prim, Ns=2e4):
+    q = dict(p)
+    q["Ns_target"] = Ns
+    q["w_min"] = wmin_per_ns(q, prim, 1e-17) / Ns
+    b0 = 1e4
+    for it in range(6):
+        q["bias0"] = b0
+        o = Oracle(q, prim)
+        o.prepare()
+        o.run()
+        s = o.stats()
+        ratio = s["n_spawned"] / max(1, s["n_primary"])
+        print(f"  bias0={b0:.4g} spawned/primaries={ratio:.3f}", flush=True)
+        if abs(ratio / SPAWN_TARGET - 1) < 0.05:
+            break
+        b0 *= SPAWN_TARGET / max(ratio, 1e-3)
+    return float(f"{b0:.3g}"), ratio
+
+
+def flux230(p, prim):
+    q = dict(p)
+    q.update(Ns_target=1e5, scattering_on=0, nu_min=1e10, nu_max=1e13, w_min=0.0)
+    o = Oracle(q, prim)
+    o.prepare()
+    o.run()
+    spec, _, _ = o.spectrum()
+    nub = q["nu_lo"] * np.exp((np.arange(q["n_nu"]) + 0.5) * math.log(q["nu_hi"] / q["nu_lo"]) / q["n_nu"])
+    j = int(np.argmin(abs(nub - 2.3e11)))
+    D = 8.1e3 * 3.085678e18
+    return float(spec[3:5, j - 1:j + 2].mean() / (4 * math.pi * D * D * nub[j]) / 1e-23)
+
+
+def main():
+    cal = {}
+    p, prim = wl.sphere(1e13, 10.0, 1.0, 1e3, 32, 16, 1e5, 1, False)
+    cal["cfg0"] = {"w_min_per_Ns1": wmin_per_ns(p, prim)}
+    print("cfg0", cal["cfg0"], flush=True)
+    n_e = 1e-2 / (wl.SIGMA_T * 1e3)
+    p, prim = wl.sphere(n_e, 4.0, 1.0, 1e3, 32, 16, 1e6, 1, True)
+    cal["cfg1"] = {"w_min_per_Ns1": wmin_per_ns(p, prim, 1e-14)}
+    print("cfg1", cal["cfg1"], flush=True)
+
+    p, prim = wl.torus(256, 256, 1, Ns=1e7, seed=1)
+    p["M_unit"] = M_UNIT_TORUS
+    b0, ratio = tune_bias(p, prim)
+    cal["cfg2"] = {"M_unit": M_UNIT_TORUS, "bias0": b0, "w_min_per_Ns1": wmin_per_ns(p, prim, 1e-17),
+                   "spawn_ratio_at_calibration": ratio, "F230_Jy_45_75deg": flux230(p, prim)}
+    print("cfg2", cal["cfg2"], flush=True)
+
+    # config 3 is calibrated on a reduced 96x64x64 version of the same recipe (the full grid takes
+    # the oracle too long); bias and floor depend on the plasma state, not on the resolution
+    p, prim = wl.torus(96, 64, 64, Ns=1e7, seed=1, perturb=True)
+    p["M_unit"] = M_UNIT_TORUS
+    b0, ratio = tune_bias(p, prim)
+    cal["cfg3"] = {"M_unit": M_UNIT_TORUS, "bias0": b0, "w_min_per_Ns1": wmin_per_ns(p, prim, 1e-17),
+                   "spawn_ratio_at_calibration": ratio}
+    print("cfg3", cal["cfg3"], flush=True)
+
+    p, prim = wl.torus(256, 256, 1, Ns=1e6, seed=1, rho_scale=1e3)
+    p["M_unit"] = M_UNIT_TORUS
+    cal["cfg4"] = {"M_unit": M_UNIT_TORUS, "bias0": 1e-12, "w_min_per_Ns1": wmin_per_ns(p, prim, 1e-17)}
+    print("cfg4", cal["cfg4"], flush=True)
+    with open(OUT, "w") as f:
+        json.dump(cal, f, indent=1)
+        f.write("\n")
+
+
+if __name__ == "__main__":
+    main()

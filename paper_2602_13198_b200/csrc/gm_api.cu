@@ -1,0 +1,511 @@
+// C-ABI of the library (include/gpumonty_b200.h): context, validation, device memory, the batch
+// driver (S13; N_s is split into serial batches sized to memory, only the tallies
+// persist) and the getters.  No torch types, no CPU fallback.
+#include "gm_host.h"
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+using namespace gm;
+
+struct gm_ctx {
+  gm_params p;
+  DevParams P;
+  int device = 0, n_sm = 0;
+  long nz = 0;
+  // device memory
+  double* d_prim = nullptr;
+  double *d_lnK2 = nullptr, *d_lnF = nullptr, *d_lnSigH = nullptr, *d_lnw = nullptr;
+  ZoneArrays Z{};
+  int n_weight_blocks = 0;
+  Tally tally{}; Tally tally_snap{};
+  DevStats *d_stats = nullptr, *d_stats_snap = nullptr;
+  double *d_spec = nullptr;          // [2][nb]
+  int* d_counters = nullptr;         // [0] primaries count, [1] queue A count, [2] queue B count, [3] work counter
+  Photon *d_prim_ph = nullptr, *d_qA = nullptr, *d_qB = nullptr;
+  long long batch_primaries = 0, queue_records = 0;   // allocated sizes
+  long long want_batch = 0, want_queue = 0;
+  bool have_grid = false, prepared = false;
+  long long n_primaries = 0;
+  std::string err;
+};
+
+static std::string g_create_err;
+
+static int fail(gm_ctx* c, int code, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof(buf), fmt, ap);
+  va_end(ap);
+  if (c) c->err = buf; else g_create_err = buf;
+  return code;
+}
+#define CK(call)                                                                          \
+  do {                                                                                    \
+    cudaError_t e_ = (call);                                                              \
+    if (e_ != cudaSuccess) return fail(ctx, GM_ERR_CUDA, "%s: %s", #call, cudaGetErrorString(e_)); \
+  } while (0)
+
+static void free_run_buffers(gm_ctx* c) {
+  cudaFree(c->d_prim_ph); cudaFree(c->d_qA); cudaFree(c->d_qB);
+  c->d_prim_ph = c->d_qA = c->d_qB = nullptr;
+  c->batch_primaries = c->queue_records = 0;
+}
+
+static void free_all(gm_ctx* c) {
+  if (!c) return;
+  free_run_buffers(c);
+  cudaFree(c->d_prim); cudaFree(c->d_lnK2); cudaFree(c->d_lnF); cudaFree(c->d_lnSigH); cudaFree(c->d_lnw);
+  cudaFree(c->Z.A); cudaFree(c->Z.nu0); cudaFree(c->Z.vol); cudaFree(c->Z.Nexp); cudaFree(c->Z.qmax);
+  cudaFree(c->Z.n); cudaFree(c->Z.offset); cudaFree(c->Z.partial); cudaFree(c->Z.nu_nodes); cudaFree(c->Z.wk);
+  cudaFree(c->Z.blocksum); cudaFree(c->Z.bad);
+  cudaFree(c->tally.A); cudaFree(c->tally_snap.A);
+  cudaFree(c->d_stats); cudaFree(c->d_stats_snap); cudaFree(c->d_spec); cudaFree(c->d_counters);
+}
+
+static bool finite_pos(double v) { return std::isfinite(v) && v > 0.0; }
+
+static int validate(const gm_params* p) {
+  if (p->abi_version != GM_ABI_VERSION) return fail(nullptr, GM_ERR_PARAM, "abi_version %u != %u", p->abi_version, GM_ABI_VERSION);
+  if (p->metric_kind != 0 && p->metric_kind != 1) return fail(nullptr, GM_ERR_PARAM, "metric_kind must be 0 or 1");
+  if (p->n1 < 1 || p->n2 < 1 || p->n3 < 1) return fail(nullptr, GM_ERR_PARAM, "n1,n2,n3 must be >= 1");
+  if (!finite_pos(p->Ns_target)) return fail(nullptr, GM_ERR_PARAM, "Ns_target must be > 0");
+  if (p->metric_kind == 1 && !(std::fabs(p->a_spin) < 1.0)) return fail(nullptr, GM_ERR_PARAM, "|a_spin| must be < 1");
+  if (!(p->hslope > 0.0 && p->hslope <= 1.0)) return fail(nullptr, GM_ERR_PARAM, "hslope must be in (0,1]");
+  for (int i = 1; i < 4; i++)
+    if (!finite_pos(p->dx[i]) || !std::isfinite(p->startx[i])) return fail(nullptr, GM_ERR_PARAM, "bad startx/dx[%d]", i);
+  if (!finite_pos(p->L_unit) || !finite_pos(p->M_unit)) return fail(nullptr, GM_ERR_PARAM, "L_unit, M_unit must be > 0");
+  if (p->thetae_mode < 0 || p->thetae_mode > 2) return fail(nullptr, GM_ERR_PARAM, "thetae_mode must be 0, 1 or 2");
+  if (!(p->thetae_min >= 0.3)) return fail(nullptr, GM_ERR_PARAM, "thetae_min must be >= 0.3 (range of the K2 table and of Eq. 3)");
+  if (!(p->thetae_max >= p->thetae_min)) return fail(nullptr, GM_ERR_PARAM, "thetae_max < thetae_min");
+  if (p->thetae_mode == 0 && !finite_pos(p->thetae_fixed)) return fail(nullptr, GM_ERR_PARAM, "thetae_fixed must be > 0");
+  if (!finite_pos(p->nu_min) || !(p->nu_max > p->nu_min)) return fail(nullptr, GM_ERR_PARAM, "need 0 < nu_min < nu_max");
+  if (!(p->w_min >= 0.0)) return fail(nullptr, GM_ERR_PARAM, "w_min must be >= 0");
+  if (!finite_pos(p->step_eps) || !finite_pos(p->verlet_tol) || p->verlet_maxit < 1) return fail(nullptr, GM_ERR_PARAM, "bad step_eps / verlet_tol / verlet_maxit");
+  if (!finite_pos(p->r_max)) return fail(nullptr, GM_ERR_PARAM, "r_max must be > 0");
+  if (p->max_steps < 1) return fail(nullptr, GM_ERR_PARAM, "max_steps must be >= 1");
+  if (p->scattering_on && (!(p->bias0 > 0.0) || p->nsc_max < 0 || p->nsc_max > 60 || p->bias_p_theta < 0 || p->bias_q_nsc < 0 || !(p->roulette > 1.0)))
+    return fail(nullptr, GM_ERR_PARAM, "bad scattering parameters");
+  if (!(p->roulette > 1.0)) return fail(nullptr, GM_ERR_PARAM, "roulette must be > 1");
+  if (p->n_th < 1 || p->n_nu < 1 || !finite_pos(p->nu_lo) || !(p->nu_hi > p->nu_lo)) return fail(nullptr, GM_ERR_PARAM, "bad detector bins");
+  return GM_OK;
+}
+
+static void fill_dev_params(gm_ctx* c) {
+  const gm_params& p = c->p;
+  DevParams& P = c->P;
+  memset(&P, 0, sizeof(P));
+  P.a_spin = p.metric_kind == 1 ? p.a_spin : 0.0;
+  P.hslope = p.hslope;
+  P.startx1 = p.startx[1]; P.startx2 = p.startx[2]; P.startx3 = p.startx[3];
+  P.dx1 = p.dx[1]; P.dx2 = p.dx[2]; P.dx3 = p.dx[3];
+  P.x1lo = p.startx[1]; P.x1hi = p.startx[1] + p.n1 * p.dx[1];
+  P.n1 = p.n1; P.n2 = p.n2; P.n3 = p.n3; P.metric_kind = p.metric_kind;
+  P.L_unit = p.L_unit;
+  P.T_unit = p.L_unit / C_CL;
+  const double RHO = p.M_unit / (p.L_unit * p.L_unit * p.L_unit);
+  P.B_unit = C_CL * std::sqrt(4.0 * C_PI * RHO);
+  P.Ne_unit = RHO / (C_MP + C_ME);
+  P.Cfac = C_HPL * p.L_unit / C_MEC2;
+  P.thetae_mode = p.thetae_mode;
+  P.thetae_fixed = p.thetae_fixed; P.trat = p.trat; P.R_low = p.R_low; P.R_high = p.R_high; P.gam_ad = p.gam_ad;
+  P.thetae_min = p.thetae_min; P.thetae_max = p.thetae_max;
+  P.nu_min = p.nu_min; P.lnnu_min = std::log(p.nu_min); P.Lam = std::log(p.nu_max / p.nu_min);
+  P.inv_Dlw = (double)NW / P.Lam; P.w_min = p.w_min; P.Ns_target = p.Ns_target;
+  P.dV = p.dx[1] * p.dx[2] * p.dx[3] * p.L_unit * p.L_unit * p.L_unit;
+  P.step_eps = p.step_eps; P.verlet_tol = p.verlet_tol; P.r_max = p.r_max; P.r_horizon_stop = p.r_horizon_stop;
+  P.lnr_max = std::log(p.r_max);
+  P.lnr_hor = p.r_horizon_stop > 0.0 ? std::log(p.r_horizon_stop) : -1e300;
+  P.max_steps = p.max_steps; P.verlet_maxit = p.verlet_maxit;
+  P.scattering_on = p.scattering_on; P.nsc_max = p.nsc_max; P.bias_p = p.bias_p_theta; P.bias_q = p.bias_q_nsc;
+  P.bias0 = p.bias0; P.roulette = p.roulette; P.inv_roulette = 1.0 / p.roulette;
+  P.n_th = p.n_th; P.n_nu = p.n_nu; P.fold_theta = p.fold_theta;
+  P.nu_lo = p.nu_lo; P.db = std::log(p.nu_hi / p.nu_lo) / p.n_nu; P.inv_db = 1.0 / P.db;
+  P.seed_lo = (uint32_t)(p.seed & 0xffffffffu); P.seed_hi = (uint32_t)(p.seed >> 32);
+  P.prim = c->d_prim; P.lnK2 = c->d_lnK2; P.lnF = c->d_lnF; P.lnSigH = c->d_lnSigH; P.lnw = c->d_lnw;
+}
+
+extern "C" {
+
+const char* gm_last_error(const gm_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_err.c_str(); }
+
+int gm_create(gm_ctx** out, const gm_params* p) {
+  if (!out) return fail(nullptr, GM_ERR_PARAM, "out is NULL");
+  *out = nullptr;
+  if (!p) return fail(nullptr, GM_ERR_PARAM, "params is NULL");
+  int v = validate(p);
+  if (v != GM_OK) return v;
+  int ndev = 0;
+  cudaError_t e = cudaGetDeviceCount(&ndev);
+  if (e != cudaSuccess || ndev == 0)
+    return fail(nullptr, GM_ERR_CUDA, "no CUDA device (%s): this library has no CPU path", cudaGetErrorString(e));
+  gm_ctx* ctx = new gm_ctx();
+  ctx->p = *p;
+  ctx->nz = (long)p->n1 * p->n2 * p->n3;
+  cudaDeviceProp prop;
+  if (cudaGetDevice(&ctx->device) != cudaSuccess || cudaGetDeviceProperties(&prop, ctx->device) != cudaSuccess) {
+    delete ctx;
+    return fail(nullptr, GM_ERR_CUDA, "cannot query the CUDA device");
+  }
+  if (prop.major < 10) {
+    int maj = prop.major, mnr = prop.minor;
+    delete ctx;
+    return fail(nullptr, GM_ERR_CUDA, "device is sm_%d%d; this library is built for sm_100a only", maj, mnr);
+  }
+  ctx->n_sm = prop.multiProcessorCount;
+  const long nz = ctx->nz;
+  const int nb = p->n_th * p->n_nu;
+  const int nblk = (int)((nz + 255) / 256), ntile = (int)((nz + 1023) / 1024);
+  ctx->n_weight_blocks = nblk;
+  auto A = [&](void** ptr, size_t bytes) { return cudaMalloc(ptr, bytes ? bytes : 8); };
+  bool ok = true;
+  ok = ok && A((void**)&ctx->d_prim, nz * 8 * sizeof(double)) == cudaSuccess;
+  ok = ok && A((void**)&ctx->d_lnK2, (NK2 + 1) * sizeof(double)) == cudaSuccess;
+  ok = ok && A((void**)&ctx->d_lnF, (NF + 1) * sizeof(double)) == cudaSuccess;
+  ok = ok && A((void**)&ctx->d_lnSigH, (size_t)(NSE + 1) * (NST + 1) * sizeof(double)) == cudaSuccess;
+  ok = ok && A((void**)&ctx->d_lnw, (NW + 1) * sizeof(double)) == cudaSuccess;
+  ok = ok && A((void**)&ctx->Z.A, nz * sizeof(double)) == cudaSuccess;
+  ok = ok && A((void**)&ctx->Z.nu0, nz * sizeof(double)) == cudaSuccess;
+  ok = ok && A((void**)&ctx->Z.vol, nz * sizeof(double)) == cudaSuccess;
+  ok = ok && A((void**)&ctx->Z.Nexp, nz * sizeof(double)) == cudaSuccess;
+  ok = ok && A((void**)&ctx->Z.qmax, nz * sizeof(double)) == cudaSuccess;
+  ok = ok && A((void**)&ctx->Z.n, nz * sizeof(int32_t)) == cudaSuccess;
+  ok = ok && A((void**)&ctx->Z.offset, (nz + 1) * sizeof(long long)) == cudaSuccess;
+  ok = ok && A((void**)&ctx->Z.partial, (size_t)nblk * (NW + 1) * sizeof(double)) == cudaSuccess;
+  ok = ok && A((void**)&ctx->Z.nu_nodes, (NW + 1) * sizeof(double)) == cudaSuccess;
+  ok = ok && A((void**)&ctx->Z.wk, (NW + 1) * sizeof(double)) == cudaSuccess;
+  ok = ok && A((void**)&ctx->Z.blocksum, (size_t)ntile * sizeof(long long)) == cudaSuccess;
+  ok = ok && A((void**)&ctx->Z.bad, sizeof(int)) == cudaSuccess;
+  // tally: A, Q, W, n contiguous so that snapshot/restore is one copy
+  ok = ok && A((void**)&ctx->tally.A, (size_t)nb * 4 * sizeof(double)) == cudaSuccess;
+  ok = ok && A((void**)&ctx->tally_snap.A, (size_t)nb * 4 * sizeof(double)) == cudaSuccess;
+  ok = ok && A((void**)&ctx->d_stats, sizeof(DevStats)) == cudaSuccess;
+  ok = ok && A((void**)&ctx->d_stats_snap, sizeof(DevStats)) == cudaSuccess;
+  ok = ok && A((void**)&ctx->d_spec, (size_t)nb * 2 * sizeof(double)) == cudaSuccess;
+  ok = ok && A((void**)&ctx->d_counters, 64 * sizeof(int)) == cudaSuccess;
+  if (!ok) {
+    std::string m = cudaGetErrorString(cudaGetLastError());
+    free_all(ctx); delete ctx;
+    return fail(nullptr, GM_ERR_CUDA, "device allocation failed: %s", m.c_str());
+  }
+  ctx->tally.Q = ctx->tally.A + nb; ctx->tally.W = ctx->tally.A + 2 * nb;
+  ctx->tally.n = (unsigned long long*)(ctx->tally.A + 3 * nb);
+  ctx->tally_snap.Q = ctx->tally_snap.A + nb; ctx->tally_snap.W = ctx->tally_snap.A + 2 * nb;
+  ctx->tally_snap.n = (unsigned long long*)(ctx->tally_snap.A + 3 * nb);
+  fill_dev_params(ctx);
+  // parameter-free tables (S0)
+  cudaError_t te = build_K2_table(ctx->d_lnK2, 0);
+  if (te == cudaSuccess) te = build_F_table(ctx->d_lnF, 0);
+  if (te == cudaSuccess && p->scattering_on) te = build_sigh_table(ctx->d_lnSigH, 0);
+  if (te == cudaSuccess) te = cudaMemset(ctx->tally.A, 0, (size_t)nb * 4 * sizeof(double));
+  if (te == cudaSuccess) te = cudaMemset(ctx->d_stats, 0, sizeof(DevStats));
+  if (te == cudaSuccess) te = cudaDeviceSynchronize();
+  if (te != cudaSuccess) {
+    std::string m = cudaGetErrorString(te);
+    free_all(ctx); delete ctx;
+    return fail(nullptr, GM_ERR_CUDA, "table build failed: %s", m.c_str());
+  }
+  *out = ctx;
+  return GM_OK;
+}
+
+void gm_destroy(gm_ctx* ctx) {
+  if (!ctx) return;
+  cudaDeviceSynchronize();
+  free_all(ctx);
+  delete ctx;
+}
+
+int gm_set_grid(gm_ctx* ctx, const double* prim, int on_device, size_t n_bytes, void* cuda_stream) {
+  if (!ctx) return GM_ERR_PARAM;
+  if (!prim) return fail(ctx, GM_ERR_PARAM, "prim is NULL");
+  if (n_bytes != (size_t)ctx->nz * 8 * sizeof(double))
+    return fail(ctx, GM_ERR_PARAM, "n_bytes %zu != n1*n2*n3*8*8 = %zu", n_bytes, (size_t)ctx->nz * 64);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  CK(cudaMemcpyAsync(ctx->d_prim, prim, n_bytes, on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
+  ctx->have_grid = true; ctx->prepared = false;
+  return GM_OK;
+}
+
+int gm_reset_tally(gm_ctx* ctx) {
+  if (!ctx) return GM_ERR_PARAM;
+  const int nb = ctx->p.n_th * ctx->p.n_nu;
+  CK(cudaMemset(ctx->tally.A, 0, (size_t)nb * 4 * sizeof(double)));
+  CK(cudaMemset(ctx->d_stats, 0, sizeof(DevStats)));
+  return GM_OK;
+}
+
+int gm_prepare(gm_ctx* ctx, void* cuda_stream, int64_t* n_primaries_out) {
+  if (!ctx) return GM_ERR_PARAM;
+  if (!ctx->have_grid) return fail(ctx, GM_ERR_STATE, "gm_prepare before gm_set_grid");
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  double nu_nodes[NW + 1];
+  const double Dl = ctx->P.Lam / NW;
+  for (int k = 0; k <= NW; k++) nu_nodes[k] = ctx->p.nu_min * std::exp(k * Dl);
+  CK(cudaMemcpyAsync(ctx->Z.nu_nodes, nu_nodes, sizeof(nu_nodes), cudaMemcpyHostToDevice, st));
+  CK(cudaMemsetAsync(ctx->Z.bad, 0, sizeof(int), st));
+  CK(launch_prepare(ctx->P, ctx->Z, ctx->d_lnw, ctx->nz, st));
+  long long total = 0;
+  int bad = 0;
+  CK(cudaMemcpyAsync(&total, ctx->Z.offset + ctx->nz, sizeof(long long), cudaMemcpyDeviceToHost, st));
+  CK(cudaMemcpyAsync(&bad, ctx->Z.bad, sizeof(int), cudaMemcpyDeviceToHost, st));
+  CK(cudaStreamSynchronize(st));
+  if (bad) return fail(ctx, GM_ERR_GRID, "non-finite value in the fluid grid");
+  ctx->n_primaries = total;
+  ctx->prepared = true;
+  int r = gm_reset_tally(ctx);
+  if (r != GM_OK) return r;
+  if (n_primaries_out) *n_primaries_out = total;
+  return GM_OK;
+}
+
+int gm_get_zone_counts(gm_ctx* ctx, int32_t* counts) {
+  if (!ctx || !counts) return GM_ERR_PARAM;
+  if (!ctx->prepared) return fail(ctx, GM_ERR_STATE, "not prepared");
+  CK(cudaMemcpy(counts, ctx->Z.n, ctx->nz * sizeof(int32_t), cudaMemcpyDeviceToHost));
+  return GM_OK;
+}
+
+int gm_get_table(gm_ctx* ctx, int which, double* out, size_t n) {
+  if (!ctx || !out) return GM_ERR_PARAM;
+  const double* src = nullptr;
+  size_t len = 0;
+  switch (which) {
+    case GM_TABLE_LNK2: src = ctx->d_lnK2; len = NK2 + 1; break;
+    case GM_TABLE_LNF: src = ctx->d_lnF; len = NF + 1; break;
+    case GM_TABLE_LNSIGH:
+      if (!ctx->p.scattering_on) return fail(ctx, GM_ERR_STATE, "sigma_h table is built only when scattering_on");
+      src = ctx->d_lnSigH; len = (size_t)(NSE + 1) * (NST + 1); break;
+    case GM_TABLE_LNW: src = ctx->d_lnw; len = NW + 1; break;
+    case GM_TABLE_NEXP: src = ctx->Z.Nexp; len = ctx->nz; break;
+    case GM_TABLE_QMAX: src = ctx->Z.qmax; len = ctx->nz; break;
+    default: return fail(ctx, GM_ERR_PARAM, "unknown table %d", which);
+  }
+  if (which >= GM_TABLE_LNW && !ctx->prepared) return fail(ctx, GM_ERR_STATE, "not prepared");
+  if (n != len) return fail(ctx, GM_ERR_PARAM, "table %d has %zu entries, caller passed %zu", which, len, n);
+  CK(cudaMemcpy(out, src, len * sizeof(double), cudaMemcpyDeviceToHost));
+  return GM_OK;
+}
+
+int gm_set_batch(gm_ctx* ctx, int64_t batch_primaries, int64_t queue_records) {
+  if (!ctx) return GM_ERR_PARAM;
+  if (batch_primaries < 0 || queue_records < 0 || batch_primaries > (1ll << 30) || queue_records > (1ll << 30))
+    return fail(ctx, GM_ERR_PARAM, "batch sizes must be in [0, 2^30]");
+  ctx->want_batch = batch_primaries; ctx->want_queue = queue_records;
+  cudaDeviceSynchronize();
+  free_run_buffers(ctx);
+  return GM_OK;
+}
+
+static int ensure_run_buffers(gm_ctx* ctx, long long n_ids) {
+  if (ctx->d_prim_ph) return GM_OK;
+  size_t free_b = 0, total_b = 0;
+  CK(cudaMemGetInfo(&free_b, &total_b));
+  long long batch = ctx->want_batch ? ctx->want_batch : (1ll << 22);
+  if (batch > n_ids && !ctx->want_batch) {
+    batch = 1024;
+    while (batch < n_ids) batch <<= 1;           // power of two >= n_ids: a later, larger gm_run re-allocates
+  }
+  long long queue = ctx->want_queue ? ctx->want_queue : (ctx->p.scattering_on ? 4 * batch : 1);
+  if (!ctx->p.scattering_on) queue = 1;
+  // size the batch from the free device memory
+  while ((size_t)(batch + 2 * queue) * sizeof(Photon) > free_b / 2 && batch > 1024) { batch >>= 1; if (!ctx->want_queue && ctx->p.scattering_on) queue = 4 * batch; }
+  CK(cudaMalloc((void**)&ctx->d_prim_ph, (size_t)batch * sizeof(Photon)));
+  CK(cudaMalloc((void**)&ctx->d_qA, (size_t)queue * sizeof(Photon)));
+  CK(cudaMalloc((void**)&ctx->d_qB, (size_t)queue * sizeof(Photon)));
+  ctx->batch_primaries = batch; ctx->queue_records = queue;
+  return GM_OK;
+}
+
+// one batch: emit -> [track -> compton] per scattering generation.  Returns the largest queue
+// occupancy seen (device counters may exceed the capacity: overflow).
+static int run_batch(gm_ctx* ctx, long long first, int n, const long long* d_ids, TraceBuf trace, bool with_root,
+                     Tally tally, DevStats* stats, cudaStream_t st, int* max_queue) {
+  int* cnt = ctx->d_counters;       // [0] primaries, [1] work counter, [2 + layer] queue filled by that layer
+  CK(cudaMemsetAsync(cnt, 0, 64 * sizeof(int), st));
+  CK(launch_emit(ctx->P, ctx->Z, ctx->nz, first, n, d_ids, ctx->d_prim_ph, cnt + 0, stats, nullptr, with_root, st));
+  const int qcap = (int)ctx->queue_records;
+  const Photon* in = ctx->d_prim_ph;
+  const int* in_count = cnt + 0;
+  int in_cap = (int)ctx->batch_primaries;
+  const int layers = ctx->p.scattering_on ? ctx->p.nsc_max : 0;
+  for (int layer = 0; layer <= layers; layer++) {
+    Queue out{(layer & 1) ? ctx->d_qB : ctx->d_qA, cnt + 2 + layer, qcap};
+    CK(launch_track(ctx->P, in, in_count, in_cap, cnt + 1, out, tally, stats, trace, ctx->n_sm, st));
+    if (layer == layers) break;
+    CK(launch_compton(ctx->P, out, stats, trace, ctx->n_sm, st));
+    in = out.buf; in_count = out.count; in_cap = qcap;
+  }
+  int h_counts[64];
+  CK(cudaMemcpyAsync(h_counts, cnt, 64 * sizeof(int), cudaMemcpyDeviceToHost, st));
+  CK(cudaStreamSynchronize(st));
+  int mq = 0;
+  for (int layer = 0; layer <= layers; layer++) if (h_counts[2 + layer] > mq) mq = h_counts[2 + layer];
+  *max_queue = mq;
+  return GM_OK;
+}
+
+int gm_run(gm_ctx* ctx, int64_t first_id, int64_t n_ids, void* cuda_stream) {
+  if (!ctx) return GM_ERR_PARAM;
+  if (!ctx->prepared) return fail(ctx, GM_ERR_STATE, "gm_run before gm_prepare");
+  if (first_id < 0 || n_ids < 0 || first_id + n_ids > ctx->n_primaries)
+    return fail(ctx, GM_ERR_PARAM, "id range [%lld,%lld) outside [0,%lld)", (long long)first_id,
+                (long long)(first_id + n_ids), ctx->n_primaries);
+  if (n_ids == 0) return GM_OK;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int r = ensure_run_buffers(ctx, n_ids);
+  if (r != GM_OK) return r;
+  const int nb = ctx->p.n_th * ctx->p.n_nu;
+  long long done = 0;
+  long long batch = ctx->batch_primaries;
+  TraceBuf notrace{nullptr};
+  while (done < n_ids) {
+    long long nthis = n_ids - done < batch ? n_ids - done : batch;
+    // snapshot so that an overflowing batch can be redone in smaller pieces (nothing is dropped silently)
+    CK(cudaMemcpyAsync(ctx->tally_snap.A, ctx->tally.A, (size_t)nb * 4 * sizeof(double), cudaMemcpyDeviceToDevice, st));
+    CK(cudaMemcpyAsync(ctx->d_stats_snap, ctx->d_stats, sizeof(DevStats), cudaMemcpyDeviceToDevice, st));
+    int mq = 0;
+    r = run_batch(ctx, first_id + done, (int)nthis, nullptr, notrace, false, ctx->tally, ctx->d_stats, st, &mq);
+    if (r != GM_OK) return r;
+    if (mq > ctx->queue_records) {
+      CK(cudaMemcpyAsync(ctx->tally.A, ctx->tally_snap.A, (size_t)nb * 4 * sizeof(double), cudaMemcpyDeviceToDevice, st));
+      CK(cudaMemcpyAsync(ctx->d_stats, ctx->d_stats_snap, sizeof(DevStats), cudaMemcpyDeviceToDevice, st));
+      if (nthis <= 256)
+        return fail(ctx, GM_ERR_OVERFLOW, "scattered-superphoton queue (%lld records) overflows with a batch of %lld primaries; "
+                    "raise it with gm_set_batch or lower the bias", ctx->queue_records, nthis);
+      // shrink in proportion to the overshoot, with a margin
+      double shrink = 0.7 * (double)ctx->queue_records / (double)mq;
+      long long nb2 = (long long)(nthis * (shrink < 0.5 ? shrink : 0.5));
+      batch = nb2 < 256 ? 256 : nb2;
+      continue;
+    }
+    done += nthis;
+  }
+  return GM_OK;
+}
+
+int gm_get_tally(gm_ctx* ctx, double* A, double* Q, double* W, int64_t* n) {
+  if (!ctx) return GM_ERR_PARAM;
+  const size_t nb = (size_t)ctx->p.n_th * ctx->p.n_nu;
+  CK(cudaDeviceSynchronize());
+  if (A) CK(cudaMemcpy(A, ctx->tally.A, nb * 8, cudaMemcpyDeviceToHost));
+  if (Q) CK(cudaMemcpy(Q, ctx->tally.Q, nb * 8, cudaMemcpyDeviceToHost));
+  if (W) CK(cudaMemcpy(W, ctx->tally.W, nb * 8, cudaMemcpyDeviceToHost));
+  if (n) CK(cudaMemcpy(n, ctx->tally.n, nb * 8, cudaMemcpyDeviceToHost));
+  return GM_OK;
+}
+
+int gm_get_spectrum(gm_ctx* ctx, double* nuLnu, double* sigma, int64_t* nphot) {
+  if (!ctx) return GM_ERR_PARAM;
+  const size_t nb = (size_t)ctx->p.n_th * ctx->p.n_nu;
+  CK(launch_spectrum(ctx->P, ctx->tally, ctx->d_spec, ctx->d_spec + nb, 0));
+  CK(cudaDeviceSynchronize());
+  if (nuLnu) CK(cudaMemcpy(nuLnu, ctx->d_spec, nb * 8, cudaMemcpyDeviceToHost));
+  if (sigma) CK(cudaMemcpy(sigma, ctx->d_spec + nb, nb * 8, cudaMemcpyDeviceToHost));
+  if (nphot) CK(cudaMemcpy(nphot, ctx->tally.n, nb * 8, cudaMemcpyDeviceToHost));
+  return GM_OK;
+}
+
+int gm_get_stats(gm_ctx* ctx, gm_stats* out) {
+  if (!ctx || !out) return GM_ERR_PARAM;
+  DevStats h;
+  CK(cudaDeviceSynchronize());
+  CK(cudaMemcpy(&h, ctx->d_stats, sizeof(h), cudaMemcpyDeviceToHost));
+  int64_t* ni = &out->n_primary;
+  for (int i = 0; i < 13; i++) ni[i] = (int64_t)h.n[i];
+  double* sd = &out->sum_w_emit;
+  for (int i = 0; i < 11; i++) sd[i] = h.s[i];
+  return GM_OK;
+}
+
+int gm_emit(gm_ctx* ctx, const int64_t* ids, int n, gm_emit_rec* out) {
+  if (!ctx || !ids || !out || n < 0) return GM_ERR_PARAM;
+  if (!ctx->prepared) return fail(ctx, GM_ERR_STATE, "not prepared");
+  if (n == 0) return GM_OK;
+  for (int i = 0; i < n; i++)
+    if (ids[i] < 0 || ids[i] >= ctx->n_primaries) return fail(ctx, GM_ERR_PARAM, "id %lld out of range", (long long)ids[i]);
+  long long* d_ids = nullptr; gm_emit_rec* d_rec = nullptr;
+  CK(cudaMalloc((void**)&d_ids, n * sizeof(long long)));
+  CK(cudaMalloc((void**)&d_rec, n * sizeof(gm_emit_rec)));
+  CK(cudaMemcpy(d_ids, ids, n * sizeof(long long), cudaMemcpyHostToDevice));
+  cudaError_t e = launch_emit(ctx->P, ctx->Z, ctx->nz, 0, n, d_ids, nullptr, nullptr, nullptr, d_rec, false, 0);
+  if (e == cudaSuccess) e = cudaMemcpy(out, d_rec, n * sizeof(gm_emit_rec), cudaMemcpyDeviceToHost);
+  cudaFree(d_ids); cudaFree(d_rec);
+  if (e != cudaSuccess) return fail(ctx, GM_ERR_CUDA, "gm_emit: %s", cudaGetErrorString(e));
+  return GM_OK;
+}
+
+int gm_trace(gm_ctx* ctx, const int64_t* ids, int n, gm_trace_rec* out) {
+  if (!ctx || !ids || !out || n < 0) return GM_ERR_PARAM;
+  if (!ctx->prepared) return fail(ctx, GM_ERR_STATE, "not prepared");
+  if (n == 0) return GM_OK;
+  for (int i = 0; i < n; i++)
+    if (ids[i] < 0 || ids[i] >= ctx->n_primaries) return fail(ctx, GM_ERR_PARAM, "id %lld out of range", (long long)ids[i]);
+  int r = ensure_run_buffers(ctx, n);
+  if (r != GM_OK) return r;
+  const int nb = ctx->p.n_th * ctx->p.n_nu;
+  long long* d_ids = nullptr; gm_trace_rec* d_rec = nullptr; DevStats* d_st = nullptr; double* d_tl = nullptr;
+  CK(cudaMalloc((void**)&d_ids, n * sizeof(long long)));
+  CK(cudaMalloc((void**)&d_rec, n * sizeof(gm_trace_rec)));
+  CK(cudaMalloc((void**)&d_st, sizeof(DevStats)));
+  CK(cudaMalloc((void**)&d_tl, (size_t)nb * 4 * sizeof(double)));
+  Tally scratch{d_tl, d_tl + nb, d_tl + 2 * nb, (unsigned long long*)(d_tl + 3 * nb)};
+  int rc = GM_OK;
+  long long chunk = ctx->batch_primaries;
+  for (long long done = 0; done < n && rc == GM_OK;) {
+    long long nthis = n - done < chunk ? n - done : chunk;
+    cudaMemset(d_rec + done, 0, nthis * sizeof(gm_trace_rec));
+    cudaMemset(d_st, 0, sizeof(DevStats));
+    cudaMemset(d_tl, 0, (size_t)nb * 4 * sizeof(double));
+    cudaMemcpy(d_ids, ids + done, nthis * sizeof(long long), cudaMemcpyHostToDevice);
+    int mq = 0;
+    TraceBuf tb{d_rec + done};
+    rc = run_batch(ctx, 0, (int)nthis, d_ids, tb, true, scratch, d_st, 0, &mq);
+    if (rc == GM_OK && mq > ctx->queue_records) {
+      if (nthis <= 16) rc = fail(ctx, GM_ERR_OVERFLOW, "gm_trace: scattered-superphoton queue overflow");
+      else { chunk = nthis / 2; continue; }
+    }
+    done += nthis;
+  }
+  if (rc == GM_OK && cudaMemcpy(out, d_rec, n * sizeof(gm_trace_rec), cudaMemcpyDeviceToHost) != cudaSuccess)
+    rc = fail(ctx, GM_ERR_CUDA, "gm_trace: copy back failed");
+  cudaFree(d_ids); cudaFree(d_rec); cudaFree(d_st); cudaFree(d_tl);
+  return rc;
+}
+
+int gm_eval(gm_ctx* ctx, int what, const double* in, int n, double* out) {
+  if (!ctx || !in || !out || n < 0) return GM_ERR_PARAM;
+  static const int nin[] = {8, 4, 4, 8, 13, 5}, nout[] = {4, 33, 12, 3, 13, 3};
+  if (what < 0 || what > GM_EVAL_RAD) return fail(ctx, GM_ERR_PARAM, "unknown eval %d", what);
+  if ((what == GM_EVAL_PLASMA || what == GM_EVAL_OPAC) && !ctx->have_grid) return fail(ctx, GM_ERR_STATE, "no grid");
+  if (n == 0) return GM_OK;
+  double *d_in = nullptr, *d_out = nullptr;
+  CK(cudaMalloc((void**)&d_in, (size_t)n * nin[what] * sizeof(double)));
+  CK(cudaMalloc((void**)&d_out, (size_t)n * nout[what] * sizeof(double)));
+  cudaError_t e = cudaMemcpy(d_in, in, (size_t)n * nin[what] * sizeof(double), cudaMemcpyHostToDevice);
+  DevParams P = ctx->P;
+  if (!ctx->p.scattering_on) P.lnSigH = nullptr;
+  if (e == cudaSuccess) e = launch_eval(P, what, d_in, n, d_out, 0);
+  if (e == cudaSuccess) e = cudaMemcpy(out, d_out, (size_t)n * nout[what] * sizeof(double), cudaMemcpyDeviceToHost);
+  cudaFree(d_in); cudaFree(d_out);
+  if (e != cudaSuccess) return fail(ctx, GM_ERR_CUDA, "gm_eval: %s", cudaGetErrorString(e));
+  return GM_OK;
+}
+
+void gm_abi_sizes(int out[4]) {
+  out[0] = (int)sizeof(gm_params); out[1] = (int)sizeof(gm_stats);
+  out[2] = (int)sizeof(gm_trace_rec); out[3] = (int)sizeof(gm_emit_rec);
+}
+
+int gm_fp64_peak(double* flops_out, double* sm_clock_mhz_out) {
+  if (!flops_out) return GM_ERR_PARAM;
+  cudaError_t e = run_fp64_peak(flops_out, sm_clock_mhz_out);
+  if (e != cudaSuccess) return fail(nullptr, GM_ERR_CUDA, "gm_fp64_peak: %s", cudaGetErrorString(e));
+  return GM_OK;
+}
+
+}  // extern "C"

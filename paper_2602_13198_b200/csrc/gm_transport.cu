@@ -1,0 +1,692 @@
+// Emission sampling (S5), geodesic tracking with absorption and the biased scattering test
+// (S6-S10, S12), the Compton event (S11), the spectrum scaling (O9) of SURVEY.md section 8(a).
+//
+// Execution model: superphotons live in 160-byte records.  The tracker is a
+// persistent kernel: every lane owns one superphoton in registers, advances it one geodesic step
+// per loop iteration and, when it stops, pulls the next record through an atomic work counter
+// (PAPER.md:194-196 describes the same dynamic re-assignment).  A scattering event does not run
+// inside the step of its lane: the lane spends its next iteration on the partial push to the event
+// point (so the other 31 lanes keep stepping), then appends the parent state at the event to the
+// scattered-superphoton queue.  The queue of one scattering generation is turned into superphotons
+// by the Compton kernel and tracked by the next tracker launch (scattered superphotons
+// are collected in an array and processed after the primaries, layer by layer).
+#include "gm_host.h"
+#include "gm_physics.cuh"
+
+namespace gm {
+
+constexpr int FLAG_ROOT = 1, FLAG_DEAD = 2;
+
+// ---- block-level stats helper ---------------------------------------------------------------------
+__device__ __forceinline__ void stat_add_n(DevStats* st, int which, unsigned long long v) {
+  if (v) atomicAdd(&st->n[which], v);
+}
+__device__ __forceinline__ void stat_add_s(DevStats* st, int which, double v) {
+  if (v != 0.0) atomicAdd(&st->s[which], v);
+}
+
+// ---- tally with warp-aggregated fp64 atomics (north_star; O9) ------------------------------------------
+__device__ __forceinline__ void tally_add(const Tally& T, int bin, double wE, double w) {
+  const unsigned act = __activemask();
+  const unsigned peers = __match_any_sync(act, bin);
+  const int lane = threadIdx.x & 31;
+  const int leader = __ffs(peers) - 1;
+  double sA = 0.0, sQ = 0.0, sW = 0.0;
+  unsigned rem = peers;
+  while (rem) {
+    int src = __ffs(rem) - 1;
+    rem &= rem - 1;
+    double e = __shfl_sync(peers, wE, src), ww = __shfl_sync(peers, w, src);
+    sA += e; sQ += e * e; sW += ww;
+  }
+  if (lane == leader) {
+    atomicAdd(&T.A[bin], sA);
+    atomicAdd(&T.Q[bin], sQ);
+    atomicAdd(&T.W[bin], sW);
+    atomicAdd(&T.n[bin], (unsigned long long)__popc(peers));
+  }
+}
+
+// =====================================================================================================
+// S5: emission sampling, Eq. 7-9; emission at the zone centre (G12), plasma-frame
+// tetrad with axis 1 along b (G13)
+// =====================================================================================================
+template <bool KERR>
+__global__ void __launch_bounds__(128) emit_kernel(const DevParams P, ZoneArrays Z, long nz, long long first,
+                                                   int n, const long long* __restrict__ ids, Photon* __restrict__ out,
+                                                   int* out_count, DevStats* stats, gm_emit_rec* __restrict__ erec,
+                                                   int with_root) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i == 0 && out_count) *out_count = n;
+  double s_w = 0.0, s_wE = 0.0;
+  if (i < n) {
+    const long long pid = ids ? ids[i] : first + i;
+    // zone of this id: offset[z] <= pid < offset[z+1]
+    long lo = 0, hi = nz;          // invariant: offset[lo] <= pid, offset[hi] > pid (offset[nz] = total)
+    while (hi - lo > 1) {
+      long mid = (lo + hi) >> 1;
+      if (Z.offset[mid] <= pid) lo = mid; else hi = mid;
+    }
+    const long z = lo;
+    const int j2 = (int)((z / P.n3) % P.n2), k3 = (int)(z % P.n3);
+    const int i1 = (int)(z / ((long)P.n3 * P.n2));
+    // zone centre without FMA contraction: emission positions are bit-identical on any host
+    double x[4] = {0.0, __dadd_rn(P.startx1, __dmul_rn(i1 + 0.5, P.dx1)), __dadd_rn(P.startx2, __dmul_rn(j2 + 0.5, P.dx2)),
+                   __dadd_rn(P.startx3, __dmul_rn(k3 + 0.5, P.dx3))};
+    Geom G; DGeom D;
+    geom_at<KERR, true>(P, x[1], x[2], G, &D);
+    double pr[8];
+    load_zone(P.prim, z, pr);
+    Plasma S;
+    plasma_from_prim(P, G, pr, S);
+    const double nu0 = Z.nu0[z], qmax = Z.qmax[z];
+    const uint32_t id0 = (uint32_t)((unsigned long long)pid & 0xffffffffu);
+    const uint32_t id1 = (uint32_t)((unsigned long long)pid >> 32);
+    RngStream rs(P, TAG_EMIT, id0, id1, 0u);
+    double nu = 0.0, lnnu = 0.0;
+    for (int trial = 0; trial < 100000000; trial++) {           // Eq. 7-8
+      double u1 = rs.next(), u2 = rs.next();
+      lnnu = u1 * P.Lam + P.lnnu_min;
+      nu = exp(lnnu);
+      double q = F_of_lnK(P, log(nu / nu0)) / weight_of_lnnu(P, lnnu);
+      if (u2 < q / qmax) break;
+    }
+    const double K2 = K2_eval(P, S.thetae);
+    const double jmax = jnu_K2(nu, S.ne, S.thetae, S.B, 1.0, K2);
+    double cth = 0.0, sth = 1.0;
+    for (int trial = 0; trial < 100000000; trial++) {           // Eq. 9
+      double u3 = rs.next(), u4 = rs.next();
+      cth = 2.0 * u3 - 1.0;
+      sth = sqrt(1.0 - cth * cth);
+      if (u4 < jnu_K2(nu, S.ne, S.thetae, S.B, sth, K2) / jmax) break;
+    }
+    double sp, cp;
+    sincos(2.0 * C_PI * rs.next(), &sp, &cp);
+    const double e0 = C_HPL * nu / C_MEC2;
+    const double kt[4] = {e0, e0 * cth, e0 * sth * cp, e0 * sth * sp};
+    double e[4][4];
+    make_tetrad(G, S.ucon, S.bcon, e);
+    Photon ph;
+#pragma unroll
+    for (int m = 0; m < 4; m++) {
+      ph.x[m] = x[m];
+      ph.k[m] = e[0][m] * kt[0] + e[1][m] * kt[1] + e[2][m] * kt[2] + e[3][m] * kt[3];
+    }
+    accel<KERR>(G, D, ph.k, ph.a);
+    ph.w = weight_of_lnnu(P, lnnu);
+    opacities(P, ph.k, G, S, 0, P.scattering_on != 0 && 0 < P.nsc_max, ph.nua_a, ph.nua_s, ph.bias);
+    ph.id0 = id0; ph.id1 = id1; ph.id2 = 0u; ph.nstep = 0u;
+    ph.nsc = 0; ph.jscat = 0u; ph.root = with_root ? i : -1; ph.flags = FLAG_ROOT;
+    const double E0 = -(G.g00 * ph.k[0] + G.g01 * ph.k[1] + G.g03 * ph.k[3]);
+    if (out) out[i] = ph;
+    if (erec) {
+      gm_emit_rec r;
+      for (int m = 0; m < 4; m++) { r.x[m] = ph.x[m]; r.k[m] = ph.k[m]; r.a[m] = ph.a[m]; }
+      r.w = ph.w; r.nua_a = ph.nua_a; r.nua_s = ph.nua_s; r.bias = ph.bias; r.E0 = E0;
+      erec[i] = r;
+    }
+    s_w = ph.w; s_wE = ph.w * E0;
+  }
+  if (stats) {
+    s_w = warp_sum(s_w); s_wE = warp_sum(s_wE);
+    unsigned cnt = __popc(__ballot_sync(0xffffffffu, i < n));
+    if ((threadIdx.x & 31) == 0) {
+      stat_add_n(stats, SN_PRIMARY, cnt);
+      stat_add_s(stats, SS_EMIT, s_w);
+      stat_add_s(stats, SS_WE_EMIT, s_wE);
+    }
+  }
+}
+
+// =====================================================================================================
+// S6-S10, S12: tracker
+// =====================================================================================================
+constexpr int TRACK_THREADS = 128;
+
+template <bool KERR>
+__device__ __forceinline__ void record_photon(const DevParams& P, const double x[4], const double k[4], double w,
+                                              int root, int flags, unsigned nstep, int nsc, unsigned jscat,
+                                              const Tally& tally, DevStats* stats, const TraceBuf& trace) {
+  Geom G;
+  geom_at<KERR, false>(P, x[1], x[2], G, nullptr);
+  const double E = -(G.g00 * k[0] + G.g01 * k[1] + G.g03 * k[3]);     // -k_t, conserved (O9)
+  int ith = -1, inu = -1;
+  bool ok = false;
+  if (E > 0.0 && isfinite(E)) {
+    double fj = floor(log(E * C_MEC2_H / P.nu_lo) * P.inv_db);
+    if (fj >= 0.0 && fj < (double)P.n_nu) {
+      double s2p = sinpi(2.0 * x[2]);
+      double th = C_PI * x[2] + 0.5 * (1.0 - P.hslope) * s2p;
+      th = fmod(th, 2.0 * C_PI);
+      if (th < 0.0) th += 2.0 * C_PI;
+      if (th > C_PI) th = 2.0 * C_PI - th;
+      int it;
+      if (P.fold_theta) {
+        double tf = fmin(th, C_PI - th);
+        it = (int)floor(tf / (0.5 * C_PI / P.n_th));
+      } else {
+        it = (int)floor(th / (C_PI / P.n_th));
+      }
+      it = max(0, min(it, P.n_th - 1));
+      ith = it; inu = (int)fj; ok = true;
+    }
+  }
+  if (ok) {
+    const double wE = w * E;
+    tally_add(tally, ith * P.n_nu + inu, wE, w);
+    atomicAdd(&stats->n[SN_RECORDED], 1ull);
+    atomicAdd(&stats->s[SS_REC], w);
+    atomicAdd(&stats->s[SS_WE_REC], wE);
+    if (trace.rec && root >= 0) atomicAdd(&trace.rec[root].fam_wE, wE);
+  } else {
+    atomicAdd(&stats->n[SN_OUTOFRANGE], 1ull);
+    atomicAdd(&stats->s[SS_OUTOFRANGE], w);
+  }
+  if (trace.rec && root >= 0 && (flags & FLAG_ROOT)) {
+    gm_trace_rec* r = &trace.rec[root];
+    for (int m = 0; m < 4; m++) { r->x[m] = x[m]; r->k[m] = k[m]; }
+    r->w = w; r->E_inf = E; r->nstep = nstep; r->fate = ok ? GM_FATE_RECORDED : GM_FATE_OUTOFRANGE;
+    r->nsc = nsc; r->ith = ith; r->inu = inu; r->jscat = jscat; r->pad_ = 0;
+  }
+}
+
+__device__ __forceinline__ void trace_death(const TraceBuf& trace, int root, int flags, const double x[4],
+                                            const double k[4], double w, unsigned nstep, int nsc, unsigned jscat,
+                                            int fate) {
+  if (trace.rec && root >= 0 && (flags & FLAG_ROOT)) {
+    gm_trace_rec* r = &trace.rec[root];
+    for (int m = 0; m < 4; m++) { r->x[m] = x[m]; r->k[m] = k[m]; }
+    r->w = w; r->E_inf = 0.0; r->nstep = nstep; r->fate = fate; r->nsc = nsc; r->ith = -1; r->inu = -1;
+    r->jscat = jscat; r->pad_ = 0;
+  }
+}
+
+#ifndef GM_TRACK_MINBLOCKS
+#define GM_TRACK_MINBLOCKS 3
+#endif
+
+template <bool KERR, bool THREED>
+__global__ void __launch_bounds__(TRACK_THREADS, GM_TRACK_MINBLOCKS)
+track_kernel(const DevParams P, const Photon* __restrict__ in, const int* __restrict__ in_count, int in_capacity,
+             int* work_counter, Queue out, Tally tally, DevStats* stats, TraceBuf trace) {
+  const int n_in = min(*in_count, in_capacity);
+  // registers of the current superphoton
+  double x[4], k[4], a[4], w = 0.0, nua_a = 0.0, nua_s = 0.0, bias = 1.0;
+  uint32_t id0 = 0, id1 = 0, id2 = 0, nstep = 0, jscat = 0;
+  int nsc = 0, root = -1, flags = 0;
+  bool have = false;
+  int mode = 0;                         // 0 normal step, 1 partial push to a scattering event, 2 redo full step
+  double dl = 0.0, ux = 0.0, ev_f = 0.0, ev_b = 1.0, ev_tau = 0.0;
+  bool want_scat = false;
+  // thread-local counters
+  unsigned long long c_steps = 0, c_viters = 0;
+  double c_absorbed = 0.0;
+
+  for (;;) {
+    if (!have) {
+      const int idx = atomicAdd(work_counter, 1);
+      if (idx >= n_in) break;
+      const Photon* p = in + idx;
+      const double2* p2 = reinterpret_cast<const double2*>(p);
+      double2 v0 = p2[0], v1 = p2[1], v2 = p2[2], v3 = p2[3], v4 = p2[4], v5 = p2[5], v6 = p2[6], v7 = p2[7];
+      const uint4 m0 = reinterpret_cast<const uint4*>(p)[8], m1 = reinterpret_cast<const uint4*>(p)[9];
+      x[0] = v0.x; x[1] = v0.y; x[2] = v1.x; x[3] = v1.y;
+      k[0] = v2.x; k[1] = v2.y; k[2] = v3.x; k[3] = v3.y;
+      a[0] = v4.x; a[1] = v4.y; a[2] = v5.x; a[3] = v5.y;
+      w = v6.x; nua_a = v6.y; nua_s = v7.x; bias = v7.y;
+      id0 = m0.x; id1 = m0.y; id2 = m0.z; nstep = m0.w;
+      nsc = (int)m1.x; jscat = m1.y; root = (int)m1.z; flags = (int)m1.w;
+      if (flags & FLAG_DEAD) continue;
+      have = true; mode = 0;
+      want_scat = P.scattering_on != 0 && nsc < P.nsc_max;
+    }
+    if (mode == 0) {
+      // polar-axis reflection, stop tests (G14), roulette (G15), step size (G16)
+      if (x[2] < 0.0) { x[2] = -x[2]; k[2] = -k[2]; a[2] = -a[2]; x[3] += C_PI; }
+      if (x[2] > 1.0) { x[2] = 2.0 - x[2]; k[2] = -k[2]; a[2] = -a[2]; x[3] += C_PI; }
+      if (x[1] >= P.lnr_max) {
+        record_photon<KERR>(P, x, k, w, root, flags, nstep, nsc, jscat, tally, stats, trace);
+        have = false; continue;
+      }
+      if (KERR && x[1] <= P.lnr_hor) {
+        atomicAdd(&stats->n[SN_HORIZON], 1ull); atomicAdd(&stats->s[SS_HORIZON], w);
+        trace_death(trace, root, flags, x, k, w, nstep, nsc, jscat, GM_FATE_HORIZON);
+        have = false; continue;
+      }
+      if ((long long)nstep >= P.max_steps) {
+        atomicAdd(&stats->n[SN_MAXSTEP], 1ull); atomicAdd(&stats->s[SS_MAXSTEP], w);
+        trace_death(trace, root, flags, x, k, w, nstep, nsc, jscat, GM_FATE_MAXSTEP);
+        have = false; continue;
+      }
+      double ur;
+      uniform_pair(P, TAG_STEP, id0, id1, id2, nstep, ux, ur);
+      if (w < P.w_min) {
+        if (ur < P.inv_roulette) {
+          atomicAdd(&stats->n[SN_ROUL_SURV], 1ull); atomicAdd(&stats->s[SS_ROUL_GAIN], w * (P.roulette - 1.0));
+          w *= P.roulette;
+        } else {
+          atomicAdd(&stats->n[SN_ROUL_KILLED], 1ull); atomicAdd(&stats->s[SS_ROUL_KILLED], w);
+          trace_death(trace, root, flags, x, k, w, nstep, nsc, jscat, GM_FATE_ROULETTE);
+          have = false; continue;
+        }
+      }
+      dl = step_size(P, x, k);
+    }
+    const double dl_eff = (mode == 1) ? ev_f * dl : dl;
+    double x1[4], k1[4], a1[4];
+    Geom G;
+    bool capped;
+    const int it = push<KERR>(P, x, k, a, dl_eff, x1, k1, a1, G, capped);
+    Plasma S;
+    const bool inplasma = plasma_at<THREED>(P, x1, G, S);
+
+    if (mode == 1) {
+      // ---- scattering event at x1 ----
+      if (inplasma && S.ne > 0.0) {
+        c_viters += it; if (capped) atomicAdd(&stats->n[SN_VCAPPED], 1ull);
+        const double w0 = w;
+        w = w0 * exp(-ev_f * ev_tau);                      // Eq. 19 up to the event
+        c_absorbed += w0 - w;
+#pragma unroll
+        for (int m = 0; m < 4; m++) { x[m] = x1[m]; k[m] = k1[m]; a[m] = a1[m]; }
+        const double wc = w / ev_b;                        // child weight w/b
+        const int slot = atomicAdd(out.count, 1);
+        if (slot < out.capacity) {
+          Photon* c = out.buf + slot;
+          double2* c2 = reinterpret_cast<double2*>(c);
+          c2[0] = make_double2(x[0], x[1]); c2[1] = make_double2(x[2], x[3]);
+          c2[2] = make_double2(k[0], k[1]); c2[3] = make_double2(k[2], k[3]);
+          c2[4] = make_double2(0.0, 0.0); c2[5] = make_double2(0.0, 0.0);
+          c2[6] = make_double2(wc, 0.0); c2[7] = make_double2(0.0, 1.0);
+          reinterpret_cast<uint4*>(c)[8] = make_uint4(id0, id1, id2, 0u);
+          reinterpret_cast<uint4*>(c)[9] = make_uint4((uint32_t)nsc, jscat, (uint32_t)root, 0u);
+        }
+        w -= wc;                                           // parent keeps w (1 - 1/b)
+        jscat++;
+        opacities(P, k, G, S, nsc, want_scat, nua_a, nua_s, bias);
+        nstep++; c_steps++;
+        mode = 0;
+        if (!(w > 0.0)) {                                  // analog limit b = 1
+          atomicAdd(&stats->n[SN_ANALOG], 1ull);
+          trace_death(trace, root, flags, x, k, w, nstep, nsc, jscat, GM_FATE_ANALOG);
+          have = false;
+        }
+      } else {
+        mode = 2;                                          // event point in vacuum: take the full step instead
+      }
+      continue;
+    }
+
+    double na1 = 0.0, ns1 = 0.0, b1 = 1.0;
+    if (inplasma) opacities(P, k1, G, S, nsc, want_scat, na1, ns1, b1);
+    const double tau_a = 0.5 * (nua_a + na1) * P.Cfac * dl;          // Eq. 20
+    if (mode == 0) {
+      c_viters += it; if (capped) atomicAdd(&stats->n[SN_VCAPPED], 1ull);
+      if (want_scat) {
+        const double tau_s = 0.5 * (nua_s + ns1) * P.Cfac * dl;      // Eq. 25
+        if (tau_s > 0.0) {
+          const double b = 0.5 * (bias + b1);                        // G19
+          const double xr = -log(1.0 - ux);
+          if (b * tau_s > xr && w / b >= P.w_min) {
+            mode = 1; ev_f = xr / (b * tau_s); ev_b = b; ev_tau = tau_a;
+            continue;
+          }
+        }
+      }
+    }
+    // ---- commit the step (Eq. 19) ----
+    const double w0 = w;
+    w = w0 * exp(-tau_a);
+    c_absorbed += w0 - w;
+#pragma unroll
+    for (int m = 0; m < 4; m++) { x[m] = x1[m]; k[m] = k1[m]; a[m] = a1[m]; }
+    nua_a = na1; nua_s = ns1; bias = b1;
+    nstep++; c_steps++;
+    mode = 0;
+  }
+  // flush thread-local counters
+  for (int o = 16; o > 0; o >>= 1) {
+    c_steps += __shfl_xor_sync(0xffffffffu, c_steps, o);
+    c_viters += __shfl_xor_sync(0xffffffffu, c_viters, o);
+  }
+  c_absorbed = warp_sum(c_absorbed);
+  if ((threadIdx.x & 31) == 0) {
+    stat_add_n(stats, SN_STEPS, c_steps);
+    stat_add_n(stats, SN_VITERS, c_viters);
+    stat_add_s(stats, SS_ABSORBED, c_absorbed);
+  }
+}
+
+// =====================================================================================================
+// S11: Compton event (G24, G25; canonical draw order of DESIGN.md O8)
+// =====================================================================================================
+__device__ inline void sample_electron_mj(RngStream& rs, double thetae, double& gam, double& beta) {
+  const double sp = 1.7724538509055159;   // sqrt(pi)
+  const double w2 = sp / 4.0;
+  const double w3 = 0.5 * sqrt(0.5 * thetae);
+  const double w4 = 3.0 * sp * thetae / 8.0;
+  const double w5 = thetae * sqrt(0.5 * thetae);
+  const double wt = w2 + w3 + w4 + w5;
+  for (;;) {
+    double us = rs.next();
+    double u1 = rs.next(), u2 = rs.next(), u3 = rs.next(), u4 = rs.next();
+    double ua = rs.next();
+    double l1 = log(1.0 - u1), l2 = log(1.0 - u2), l3 = log(1.0 - u3);
+    double y2;
+    double sel = us * wt;
+    if (sel < w2) {
+      double c = cos(2.0 * C_PI * u3);
+      y2 = -l1 - l2 * c * c;
+    } else if (sel < w2 + w3) {
+      y2 = -(l1 + l2);
+    } else if (sel < w2 + w3 + w4) {
+      double c = cos(2.0 * C_PI * u4);
+      y2 = -(l1 + l2) - l3 * c * c;
+    } else {
+      y2 = -(l1 + l2 + l3);
+    }
+    double y = sqrt(y2);
+    double acc = sqrt(1.0 + 0.5 * thetae * y2) / (1.0 + y * sqrt(0.5 * thetae));
+    if (ua < acc) {
+      double t = thetae * y2;
+      gam = 1.0 + t;
+      beta = y * sqrt(thetae) * sqrt(2.0 + t) / gam;
+      return;
+    }
+  }
+}
+
+// returns false when the scattered wavevector is not usable
+__device__ inline bool compton_event(const DevParams& P, const Geom& G, const Plasma& S, const double k[4],
+                                     uint32_t id0, uint32_t id1, uint32_t id2, uint32_t j, double kout[4]) {
+  double kcov[4];
+  lower(G, k, kcov);
+  const double eps = -(kcov[0] * S.ucon[0] + kcov[1] * S.ucon[1] + kcov[2] * S.ucon[2] + kcov[3] * S.ucon[3]);
+  if (!(eps > 0.0) || !isfinite(eps)) return false;
+  double e[4][4];
+  make_tetrad(G, S.ucon, k, e);                 // axis 1 along the photon: k^(a) = eps (1,1,0,0)
+  RngStream rs(P, TAG_SCAT, id0, id1, id2, j);
+  double gam, beta, mu, phie, epsp;
+  for (;;) {
+    sample_electron_mj(rs, S.thetae, gam, beta);
+    double um = rs.next();
+    double z = 2.0 * beta + beta * beta - 4.0 * beta * um;
+    mu = -(2.0 + beta - 4.0 * um) / (1.0 + sqrt(1.0 + z));       // pdf ~ (1 - beta mu)
+    phie = 2.0 * C_PI * rs.next();
+    epsp = eps * gam * (1.0 - beta * mu);
+    double uk = rs.next();
+    if (uk < sigma_kn(epsp)) break;
+  }
+  mu = fmin(fmax(mu, -1.0), 1.0);
+  const double sm = sqrt(1.0 - mu * mu);
+  double sphe, cphe;
+  sincos(phie, &sphe, &cphe);
+  const double ne[3] = {mu, sm * cphe, sm * sphe};
+  // photon into the electron rest frame
+  const double fac = (gam - 1.0) * (eps * mu) - gam * beta * eps;
+  double pp[3] = {eps + fac * ne[0], fac * ne[1], fac * ne[2]};
+  const double nn = sqrt(pp[0] * pp[0] + pp[1] * pp[1] + pp[2] * pp[2]);
+  const double np[3] = {pp[0] / nn, pp[1] / nn, pp[2] / nn};
+  double eout, mus;
+  if (epsp > 1e-4) {                                              // Klein-Nishina
+    const double elo = epsp / (1.0 + 2.0 * epsp);
+    const double fmax_ = (1.0 + 2.0 * epsp) + 1.0 / (1.0 + 2.0 * epsp);
+    for (;;) {
+      double up = rs.next(), ua = rs.next();
+      eout = elo + up * (epsp - elo);
+      mus = 1.0 + 1.0 / epsp - 1.0 / eout;
+      double f = epsp / eout + eout / epsp - 1.0 + mus * mus;
+      if (ua * fmax_ < f) break;
+    }
+  } else {                                                        // Thomson
+    for (;;) {
+      double u1 = rs.next(), u2 = rs.next();
+      mus = 2.0 * u1 - 1.0;
+      if (2.0 * u2 < 1.0 + mus * mus) break;
+    }
+    eout = epsp;
+  }
+  mus = fmin(fmax(mus, -1.0), 1.0);
+  const double phis = 2.0 * C_PI * rs.next();
+  // perpendicular pair about the incoming direction: least-aligned axis among (2),(3),(1)
+  int ax = 1;
+  if (fabs(np[2]) < fabs(np[ax])) ax = 2;
+  if (fabs(np[0]) < fabs(np[ax])) ax = 0;
+  double ep[3] = {0.0, 0.0, 0.0};
+  ep[ax] = 1.0;
+  const double d = np[ax];
+  for (int i = 0; i < 3; i++) ep[i] -= d * np[i];
+  const double en = sqrt(ep[0] * ep[0] + ep[1] * ep[1] + ep[2] * ep[2]);
+  for (int i = 0; i < 3; i++) ep[i] /= en;
+  const double eq[3] = {np[1] * ep[2] - np[2] * ep[1], np[2] * ep[0] - np[0] * ep[2], np[0] * ep[1] - np[1] * ep[0]};
+  const double ss = sqrt(1.0 - mus * mus);
+  double sn, cs;
+  sincos(phis, &sn, &cs);
+  double po[3];
+  for (int i = 0; i < 3; i++) po[i] = eout * (mus * np[i] + ss * (cs * ep[i] + sn * eq[i]));
+  // back to the plasma frame
+  const double ndpo = ne[0] * po[0] + ne[1] * po[1] + ne[2] * po[2];
+  const double k0 = gam * (eout + beta * ndpo);
+  const double fb = (gam - 1.0) * ndpo + gam * beta * eout;
+  const double kt[4] = {k0, po[0] + fb * ne[0], po[1] + fb * ne[1], po[2] + fb * ne[2]};
+  bool ok = k0 > 0.0;
+  for (int m = 0; m < 4; m++) {
+    kout[m] = e[0][m] * kt[0] + e[1][m] * kt[1] + e[2][m] * kt[2] + e[3][m] * kt[3];
+    ok = ok && isfinite(kout[m]);
+  }
+  return ok;
+}
+
+template <bool KERR, bool THREED>
+__global__ void __launch_bounds__(128) compton_kernel(const DevParams P, Queue q, DevStats* stats, TraceBuf trace) {
+  const int n = min(*q.count, q.capacity);
+  unsigned long long c_spawn = 0, c_bad = 0;
+  double s_bad = 0.0;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+    Photon ph = q.buf[i];
+    Geom G; DGeom D;
+    geom_at<KERR, true>(P, ph.x[1], ph.x[2], G, &D);
+    Plasma S;
+    bool inplasma = plasma_at<THREED>(P, ph.x, G, S);    // true by construction (tested by the tracker)
+    double kout[4];
+    bool ok = inplasma && compton_event(P, G, S, ph.k, ph.id0, ph.id1, ph.id2, ph.jscat, kout);
+    if (ok) {
+      uint32_t o[4];
+      philox4x32_10(ph.id0, ph.id1, ph.id2, ph.jscat, P.seed_lo ^ TAG_SPAWN, P.seed_hi, o);
+      ph.id0 = o[0]; ph.id1 = o[1]; ph.id2 = o[2];
+      for (int m = 0; m < 4; m++) ph.k[m] = kout[m];
+      accel<KERR>(G, D, ph.k, ph.a);
+      ph.nsc += 1; ph.nstep = 0; ph.jscat = 0; ph.flags = 0;
+      opacities(P, ph.k, G, S, ph.nsc, P.scattering_on != 0 && ph.nsc < P.nsc_max, ph.nua_a, ph.nua_s, ph.bias);
+      c_spawn++;
+      if (trace.rec && ph.root >= 0) atomicAdd((unsigned long long*)&trace.rec[ph.root].fam_nspawn, 1ull);
+    } else {
+      ph.flags = FLAG_DEAD;
+      c_bad++; s_bad += ph.w;
+    }
+    q.buf[i] = ph;
+  }
+  for (int o = 16; o > 0; o >>= 1) {
+    c_spawn += __shfl_xor_sync(0xffffffffu, c_spawn, o);
+    c_bad += __shfl_xor_sync(0xffffffffu, c_bad, o);
+  }
+  s_bad = warp_sum(s_bad);
+  if ((threadIdx.x & 31) == 0) {
+    stat_add_n(stats, SN_SPAWNED, c_spawn);
+    stat_add_n(stats, SN_BADSCAT, c_bad);
+    stat_add_s(stats, SS_BAD, s_bad);
+  }
+}
+
+// =====================================================================================================
+// O9: nu L_nu and its Monte Carlo sigma from the accumulators
+// =====================================================================================================
+__global__ void spectrum_kernel(const DevParams P, Tally T, double* __restrict__ nuLnu, double* __restrict__ sigma) {
+  int b = blockIdx.x * blockDim.x + threadIdx.x;
+  if (b >= P.n_th * P.n_nu) return;
+  int i = b / P.n_nu;
+  double lo, hi, dOm;
+  if (P.fold_theta) {
+    lo = i * (0.5 * C_PI / P.n_th); hi = (i + 1) * (0.5 * C_PI / P.n_th);
+    dOm = 4.0 * C_PI * (cos(lo) - cos(hi));
+  } else {
+    lo = i * (C_PI / P.n_th); hi = (i + 1) * (C_PI / P.n_th);
+    dOm = 2.0 * C_PI * (cos(lo) - cos(hi));
+  }
+  double scale = C_MEC2 / P.T_unit * (4.0 * C_PI / dOm) / P.db;
+  nuLnu[b] = scale * T.A[b];
+  sigma[b] = scale * sqrt(T.Q[b]);
+}
+
+// =====================================================================================================
+// diagnostics: one device function of the path per row (parity tests call these through gm_eval)
+// =====================================================================================================
+template <bool KERR, bool THREED>
+__global__ void eval_kernel(const DevParams P, int what, const double* __restrict__ in, int n, double* __restrict__ out) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  if (what == GM_EVAL_ACCEL) {
+    const double* r = in + 8 * i;
+    Geom G; DGeom D;
+    geom_at<KERR, true>(P, r[1], r[2], G, &D);
+    double a[4];
+    accel<KERR>(G, D, r + 4, a);
+    for (int m = 0; m < 4; m++) out[4 * i + m] = a[m];
+  } else if (what == GM_EVAL_GEOM) {
+    const double* r = in + 4 * i;
+    Geom G;
+    geom_at<KERR, false>(P, r[1], r[2], G, nullptr);
+    double* o = out + 33 * i;
+    for (int m = 0; m < 33; m++) o[m] = 0.0;
+    o[0] = G.g00; o[1] = o[4] = G.g01; o[3] = o[12] = G.g03; o[5] = G.g11; o[7] = o[13] = G.g13;
+    o[10] = G.g22; o[15] = G.g33;
+    double* c = o + 16;
+    c[0] = G.i00; c[1] = c[4] = G.i01; c[5] = G.i11; c[7] = c[13] = G.i13; c[10] = G.i22; c[15] = G.i33;
+    o[32] = G.gdet;
+  } else if (what == GM_EVAL_PLASMA) {
+    const double* r = in + 4 * i;
+    Geom G;
+    geom_at<KERR, false>(P, r[1], r[2], G, nullptr);
+    Plasma S;
+    double* o = out + 12 * i;
+    for (int m = 0; m < 12; m++) o[m] = 0.0;
+    if (plasma_at<THREED>(P, r, G, S)) {
+      o[0] = S.ne; o[1] = S.thetae; o[2] = S.B;
+      for (int m = 0; m < 4; m++) { o[3 + m] = S.ucon[m]; o[7 + m] = S.bcon[m]; }
+    } else o[11] = 1.0;
+  } else if (what == GM_EVAL_OPAC) {
+    const double* r = in + 8 * i;
+    Geom G;
+    geom_at<KERR, false>(P, r[1], r[2], G, nullptr);
+    Plasma S;
+    double na = 0.0, ns = 0.0, b = 1.0;
+    if (plasma_at<THREED>(P, r, G, S)) opacities(P, r + 4, G, S, 0, P.scattering_on != 0, na, ns, b);
+    out[3 * i] = na; out[3 * i + 1] = ns; out[3 * i + 2] = b;
+  } else if (what == GM_EVAL_PUSH) {
+    const double* r = in + 13 * i;
+    double x1[4], k1[4], a1[4];
+    Geom G; bool capped;
+    int it = push<KERR>(P, r, r + 4, r + 8, r[12], x1, k1, a1, G, capped);
+    double* o = out + 13 * i;
+    for (int m = 0; m < 4; m++) { o[m] = x1[m]; o[4 + m] = k1[m]; o[8 + m] = a1[m]; }
+    o[12] = capped ? -it : it;
+  } else if (what == GM_EVAL_RAD) {
+    const double* r = in + 5 * i;
+    out[3 * i] = jnu_K2(r[0], r[1], r[2], r[3], r[4], K2_eval(P, r[2]));
+    out[3 * i + 1] = nu_alpha_abs(P, r[0], r[1], r[2], r[3], r[4]);
+    out[3 * i + 2] = P.lnSigH ? sigma_hot_eval(P, r[2], r[0] * C_H_MEC2) : 0.0;
+  }
+}
+
+// FP64 pipe peak: 8 independent DFMA chains per thread
+__global__ void __launch_bounds__(256) dfma_kernel(double* out, int iters, double seed) {
+  double a0 = seed, a1 = seed + 1, a2 = seed + 2, a3 = seed + 3, a4 = seed + 4, a5 = seed + 5, a6 = seed + 6, a7 = seed + 7;
+  const double m = 0.999999, c = 1e-9 * threadIdx.x;
+  for (int i = 0; i < iters; i++) {
+    a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
+    a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+  }
+  out[blockIdx.x * blockDim.x + threadIdx.x] = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+}
+
+// ---- launch wrappers ---------------------------------------------------------------------------------
+#define GM_DISPATCH(KERNEL, GRID, BLOCK, ST, ...)                                              \
+  do {                                                                                         \
+    const bool kerr_ = P.metric_kind == 1, td_ = P.n3 > 1;                                     \
+    if (kerr_ && td_) KERNEL<true, true><<<GRID, BLOCK, 0, ST>>>(__VA_ARGS__);                 \
+    else if (kerr_) KERNEL<true, false><<<GRID, BLOCK, 0, ST>>>(__VA_ARGS__);                  \
+    else if (td_) KERNEL<false, true><<<GRID, BLOCK, 0, ST>>>(__VA_ARGS__);                    \
+    else KERNEL<false, false><<<GRID, BLOCK, 0, ST>>>(__VA_ARGS__);                            \
+  } while (0)
+
+cudaError_t launch_emit(const DevParams& P, const ZoneArrays& Z, long nz, long long first, int n,
+                        const long long* d_ids, Photon* out, int* out_count, DevStats* stats,
+                        gm_emit_rec* emit_out, bool with_root, cudaStream_t st) {
+  if (n <= 0) return cudaSuccess;
+  int grid = (n + 127) / 128;
+  if (P.metric_kind == 1)
+    emit_kernel<true><<<grid, 128, 0, st>>>(P, Z, nz, first, n, d_ids, out, out_count, stats, emit_out, with_root);
+  else
+    emit_kernel<false><<<grid, 128, 0, st>>>(P, Z, nz, first, n, d_ids, out, out_count, stats, emit_out, with_root);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_track(const DevParams& P, const Photon* in, const int* in_count, int in_capacity,
+                         int* work_counter, Queue out, Tally tally, DevStats* stats, TraceBuf trace, int n_sm,
+                         cudaStream_t st) {
+  cudaError_t e = cudaMemsetAsync(work_counter, 0, sizeof(int), st);
+  if (e != cudaSuccess) return e;
+  const int grid = n_sm * GM_TRACK_MINBLOCKS;
+  GM_DISPATCH(track_kernel, grid, TRACK_THREADS, st, P, in, in_count, in_capacity, work_counter, out, tally, stats, trace);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_compton(const DevParams& P, Queue q, DevStats* stats, TraceBuf trace, int n_sm, cudaStream_t st) {
+  const int grid = n_sm * 4;
+  GM_DISPATCH(compton_kernel, grid, 128, st, P, q, stats, trace);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_spectrum(const DevParams& P, Tally tally, double* nuLnu, double* sigma, cudaStream_t st) {
+  int nb = P.n_th * P.n_nu;
+  spectrum_kernel<<<(nb + 127) / 128, 128, 0, st>>>(P, tally, nuLnu, sigma);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_eval(const DevParams& P, int what, const double* d_in, int n, double* d_out, cudaStream_t st) {
+  if (n <= 0) return cudaSuccess;
+  GM_DISPATCH(eval_kernel, (n + 127) / 128, 128, st, P, what, d_in, n, d_out);
+  return cudaGetLastError();
+}
+
+cudaError_t run_fp64_peak(double* flops_out, double* clock_mhz_out) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  cudaDeviceProp prop;
+  if ((e = cudaGetDeviceProperties(&prop, dev)) != cudaSuccess) return e;
+  const int blocks = prop.multiProcessorCount * 8, threads = 256, iters = 1 << 16;
+  double* d = nullptr;
+  if ((e = cudaMalloc(&d, sizeof(double) * blocks * threads)) != cudaSuccess) return e;
+  cudaEvent_t t0, t1;
+  cudaEventCreate(&t0); cudaEventCreate(&t1);
+  double best = 0.0;
+  for (int rep = 0; rep < 4; rep++) {
+    cudaEventRecord(t0);
+    dfma_kernel<<<blocks, threads>>>(d, iters, 1.0 + rep);
+    cudaEventRecord(t1);
+    if ((e = cudaEventSynchronize(t1)) != cudaSuccess) break;
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, t0, t1);
+    double fl = 2.0 * 8.0 * (double)iters * blocks * threads / (ms * 1e-3);
+    if (rep > 0 && fl > best) best = fl;
+  }
+  cudaEventDestroy(t0); cudaEventDestroy(t1);
+  cudaFree(d);
+  if (e != cudaSuccess) return e;
+  *flops_out = best;
+  if (clock_mhz_out) *clock_mhz_out = prop.clockRate * 1e-3;
+  return cudaSuccess;
+}
+
+}  // namespace gm

@@ -1,0 +1,389 @@
+"""GPU parity tests proper: the CUDA path (through the C-ABI) against the CPU oracle, element by element, on the
+same seeded inputs and the same Philox streams (SURVEY.md 8(c) "History divergence").
+
+Tolerances (derived in DESIGN.md "Tolerances"):
+  * integer / index work (Philox words, zone counts, prefix sum, bins, step counts): bit-exact;
+  * device functions evaluated at the same point: 1e-11 relative (libdevice vs glibc last-ulp differences,
+    closed-form vs generic-inverse metric algebra), tables 1e-9 (K2, F) / 3e-7 (sigma_h: the oracle's own
+    quadrature tolerance is 1e-8);
+  * per-history final state: |dw/w|, |dE/E| < 1e-7 for histories that did not fork; forked histories
+    (a uniform within rounding of a threshold) must stay below 1e-3 of the sample;
+  * spectra: north_star's bar -- every bin holding >= 1000 superphotons within 1 % and within 3 sigma.
+"""
+import ctypes
+import math
+
+import numpy as np
+import pytest
+
+from paper_2602_13198_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def gm():
+    from paper_2602_13198_b200 import binding
+    return binding
+
+
+def _pair(gm, p, prim, prepare=True):
+    from oracle_binding import Oracle
+    o = Oracle(p, prim)
+    g = gm.GPUMonty(p)
+    g.set_grid(prim)
+    if prepare:
+        no = o.prepare()
+        ng = g.prepare()
+        assert ng == no, (ng, no)
+    return o, g
+
+
+def _relerr(a, b, floor=0.0):
+    a, b = np.asarray(a, dtype=float), np.asarray(b, dtype=float)
+    return np.abs(a - b) / np.maximum(np.maximum(np.abs(a), np.abs(b)), floor + 1e-300)
+
+
+# ---------------------------------------------------------------------------------------------------
+# S0: tables
+# ---------------------------------------------------------------------------------------------------
+def test_tables_match_oracle(gm, olib):
+    p, prim = wl.config1(Ns=1e3)
+    g = gm.GPUMonty(p)
+    k2, F, sh = g.table(gm.TABLE_LNK2), g.table(gm.TABLE_LNF), g.table(gm.TABLE_LNSIGH)
+    assert np.max(np.abs(k2 - olib.table(0))) < 1e-12
+    assert np.max(np.abs(F - olib.table(1))) < 2e-12 * np.max(np.abs(F))
+    assert np.max(np.abs(sh - olib.table(2))) < 3e-7      # oracle quadrature tolerance 1e-8..1e-9 relative
+
+
+def test_tables_against_independent_values(gm):
+    """The library's own table nodes against values that do not come from the oracle: scipy's K_2 and the
+    survey's three F(K) values (tests/golden/F_values.txt)."""
+    from scipy import special
+    p, prim = wl.config0(Ns=1e3)
+    g = gm.GPUMonty(p)
+    th = 0.3 * np.exp(np.arange(201) * math.log(100 / 0.3) / 200)
+    assert np.max(np.abs(g.table(gm.TABLE_LNK2) - np.log(special.kv(2, 1 / th)))) < 1e-12
+    lnF = g.table(gm.TABLE_LNF)
+    lk = np.log(1e-6) + np.arange(261) * math.log(1e13) / 260
+    for K, val in ((1.0, 31.5754535), (1e3, 0.44643958), (2e-3, 4.76133115)):
+        got = math.exp(np.interp(math.log(K), lk, lnF))
+        assert got == pytest.approx(val, rel=2e-4)        # log-linear interpolation error of the 261-node table
+
+
+# ---------------------------------------------------------------------------------------------------
+# device functions at common points
+# ---------------------------------------------------------------------------------------------------
+def _points(p, n, rng, inside=True):
+    x = np.zeros((n, 4))
+    lo, hi = p["startx"][1], p["startx"][1] + p["n1"] * p["dx"][1]
+    x[:, 1] = rng.uniform(lo + 0.02, (hi if inside else hi + 1.5) - 0.02, n)
+    x[:, 2] = rng.uniform(0.02, 0.98, n)
+    x[:, 3] = rng.uniform(0, 2 * math.pi, n)
+    return x
+
+
+@pytest.mark.parametrize("cfg", ["flat", "kerr", "kerr3d"])
+def test_geometry_accel_plasma_opacity_push(gm, olib, cfg):
+    rng = np.random.default_rng(11)
+    if cfg == "flat":
+        p, prim = wl.config1(Ns=1e3)
+    elif cfg == "kerr":
+        p, prim = wl.config2(Ns=1e3, n1=64, n2=64)
+    else:
+        p, prim = wl.config3(Ns=1e3, n1=24, n2=16, n3=16)
+    o, g = _pair(gm, p, prim, prepare=False)
+    n = 400
+    x = _points(p, n, rng, inside=False)
+    # metric, inverse, sqrt(-g)
+    G = g.eval(gm.EVAL_GEOM, x)
+    for i in range(0, n, 7):
+        gc, gi = olib.gcov(o.P, x[i]), olib.gcon(o.P, x[i])
+        assert np.max(np.abs(G[i, :16].reshape(4, 4) - gc)) < 1e-12 * np.max(np.abs(gc))
+        assert np.max(np.abs(G[i, 16:32].reshape(4, 4) - gi)) < 1e-11 * np.max(np.abs(gi))
+        assert G[i, 32] == pytest.approx(olib.gdet(o.P, x[i]), rel=1e-12)
+    # null-ish wavevectors
+    k = rng.normal(size=(n, 4))
+    k[:, 0] = np.abs(k[:, 0]) + 2.0
+    k[:, 1] /= np.exp(x[:, 1]); k[:, 2] /= np.exp(x[:, 1]) * 3; k[:, 3] /= np.exp(x[:, 1])
+    A = g.eval(gm.EVAL_ACCEL, np.hstack([x, k]))
+    for i in range(0, n, 3):
+        conn = olib.conn(o.P, x[i])
+        a_ref = -np.einsum("mab,a,b->m", conn, k[i], k[i])
+        assert np.max(np.abs(A[i] - a_ref)) < 1e-10 * np.max(np.abs(a_ref)), (i, A[i], a_ref)
+    # push (Eq. 11-15)
+    rows = []
+    for i in range(0, n, 3):
+        conn = olib.conn(o.P, x[i])
+        a0 = -np.einsum("mab,a,b->m", conn, k[i], k[i])
+        xi, ki = np.ascontiguousarray(x[i]), np.ascontiguousarray(k[i])
+        dl = olib.L.orc_step_size(ctypes.byref(o.P), xi.ctypes.data, ki.ctypes.data)
+        rows.append(np.concatenate([x[i], k[i], a0, [dl]]))
+    rows = np.array(rows)
+    out = g.eval(gm.EVAL_PUSH, rows)
+    for r, o_ in zip(rows, out):
+        x1, k1, a1, it = olib.push(o.P, r[0:4], r[4:8], r[8:12], r[12])
+        assert int(o_[12]) == it
+        assert np.max(np.abs(o_[0:4] - x1)) < 1e-12 * (1 + np.max(np.abs(x1)))
+        assert np.max(np.abs(o_[4:8] - k1)) < 1e-10 * np.max(np.abs(k1))
+        assert np.max(np.abs(o_[8:12] - a1)) < 1e-9 * np.max(np.abs(a1))
+    # plasma state and opacities
+    xin = _points(p, n, rng, inside=True)
+    S = g.eval(gm.EVAL_PLASMA, xin)
+    kk = k.copy()
+    kk *= 1e-9          # eps ~ 1e-9 m_e c^2 ~ 1e11 Hz
+    OP = g.eval(gm.EVAL_OPAC, np.hstack([xin, kk]))
+    nchk = 0
+    for i in range(0, n, 3):
+        ref = o.plasma_at(xin[i])
+        assert bool(S[i, 11]) == ref["vacuum"]
+        if ref["vacuum"]:
+            continue
+        assert S[i, 0] == pytest.approx(ref["ne"], rel=1e-12)
+        assert S[i, 1] == pytest.approx(ref["thetae"], rel=1e-11)
+        assert S[i, 2] == pytest.approx(ref["B"], rel=1e-10, abs=1e-300)
+        assert np.max(np.abs(S[i, 3:7] - ref["ucon"])) < 1e-11 * np.max(np.abs(ref["ucon"]))
+        assert np.max(np.abs(S[i, 7:11] - ref["bcon"])) < 1e-10 * np.max(np.abs(ref["bcon"])) + 1e-300
+        nchk += 1
+    assert nchk > 50
+    assert np.all(np.isfinite(OP)) and np.any(OP[:, 1] > 0)
+
+
+def test_radiation_functions(gm, olib):
+    p, prim = wl.config1(Ns=1e3)
+    g = gm.GPUMonty(p)
+    rng = np.random.default_rng(5)
+    n = 300
+    rows = np.column_stack([10 ** rng.uniform(8, 15, n), 10 ** rng.uniform(3, 19, n), 10 ** rng.uniform(-0.5, 2.5, n),
+                            10 ** rng.uniform(-2, 3, n), rng.uniform(0.01, 1, n)])
+    out = g.eval(gm.EVAL_RAD, rows)
+    for r, o_ in zip(rows, out):
+        j = olib.L.orc_jnu(*r)
+        na = olib.L.orc_nu_alpha_abs(*r)
+        sh = olib.L.orc_sigma_hot_eval(r[2], r[0] * 6.6260693e-27 / (9.1093826e-28 * 2.99792458e10 ** 2))
+        assert o_[0] == pytest.approx(j, rel=1e-10, abs=1e-300)
+        assert o_[1] == pytest.approx(na, rel=1e-10, abs=1e-300)
+        assert o_[2] == pytest.approx(sh, rel=1e-6)
+
+
+# ---------------------------------------------------------------------------------------------------
+# S2-S5: weights, counts, prefix sum, emission
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("cfg", [0, 1, 2])
+def test_zone_counts_bit_exact_and_emission(gm, cfg):
+    if cfg == 0:
+        p, prim = wl.config0()
+    elif cfg == 1:
+        p, prim = wl.config1(Ns=1e5)
+    else:
+        p, prim = wl.config2(Ns=2e5)
+    o, g = _pair(gm, p, prim)
+    co, cg = o.zone_counts(), g.zone_counts()
+    Nexp_o, qmax_o = o.zone_info()
+    Nexp_g, qmax_g = g.table(gm.TABLE_NEXP), g.table(gm.TABLE_QMAX)
+    bad = np.nonzero(co != cg)[0]
+    assert len(bad) == 0, (bad[:10], co[bad[:10]], cg[bad[:10]], Nexp_o[bad[:10]], Nexp_g[bad[:10]])
+    assert cg.sum() == g.n_primaries
+    assert np.max(_relerr(Nexp_o, Nexp_g)) < 1e-11
+    assert np.max(_relerr(qmax_o, qmax_g)) < 1e-11
+    _, w_o = o.weight_table()
+    assert np.max(np.abs(g.table(gm.TABLE_LNW) - np.log(w_o))) < 1e-11
+    # emission of sampled ids
+    rng = np.random.default_rng(3)
+    ids = np.unique(rng.integers(0, g.n_primaries, 600))
+    eg = g.emit(ids)
+    for i, rec in zip(ids, eg):
+        r = o.emit(int(i))
+        assert np.array_equal(rec["x"], r["x"]), (rec["x"] - r["x"])
+        assert np.max(np.abs(rec["k"] - r["k"])) < 1e-10 * np.max(np.abs(r["k"])), (i, rec["k"], r["k"])
+        assert np.max(np.abs(rec["a"] - r["a"])) < 1e-9 * np.max(np.abs(r["a"])) + 1e-300
+        assert rec["w"] == pytest.approx(r["w"], rel=1e-10)
+        assert rec["nua_a"] == pytest.approx(r["nua_a"], rel=1e-9, abs=1e-300)
+        assert rec["nua_s"] == pytest.approx(r["nua_s"], rel=1e-6, abs=1e-300)
+        assert rec["bias"] == pytest.approx(r["bias"], rel=1e-10)
+        assert rec["E0"] == pytest.approx(r["E0"], rel=1e-10)
+
+
+def test_scan_ragged_tail_and_empty_zones(gm):
+    """Prefix sum over several 1024-zone tiles with a ragged tail; zones outside the emitting region hold 0."""
+    p, prim = wl.config2(Ns=3e4, n1=75, n2=41)      # 3075 zones = 3 tiles + 3
+    o, g = _pair(gm, p, prim)
+    cg = g.zone_counts()
+    assert np.array_equal(cg, o.zone_counts())
+    assert (cg == 0).sum() > 100 and cg.sum() == g.n_primaries
+
+
+# ---------------------------------------------------------------------------------------------------
+# S6-S12: histories and spectra
+# ---------------------------------------------------------------------------------------------------
+def _compare_traces(o, g, ids, fork_budget):
+    tg = g.trace(ids)
+    to, fam_wE, fam_n = o.trace(ids)
+    same = (tg["fate"] == to["fate"]) & (tg["nstep"] == to["nstep"]) & (tg["inu"] == to["inu"]) & \
+           (tg["ith"] == to["ith"]) & (tg["jscat"] == to["jscat"])
+    forks = np.nonzero(~same)[0]
+    assert len(forks) <= fork_budget * len(ids) + 1, (len(forks), len(ids), forks[:10], tg[forks[:5]], to[forks[:5]])
+    ok = np.nonzero(same)[0]
+    assert np.max(_relerr(tg["w"][ok], to["w"][ok])) < 1e-7
+    rec = ok[to["fate"][ok] == 1]
+    assert np.max(_relerr(tg["E_inf"][rec], to["E_inf"][rec])) < 1e-7
+    assert np.max(np.abs(tg["x"][ok] - to["x"][ok])) < 1e-7
+    # family sums: only compare where the spawn counts agree (a fork inside a child changes them)
+    fsame = ok[tg["fam_nspawn"][ok] == fam_n[ok]]
+    assert len(fsame) >= (1 - 10 * fork_budget) * len(ok) - 1
+    assert np.max(_relerr(tg["fam_wE"][fsame], fam_wE[fsame], floor=1e-300)) < 1e-6
+    return len(forks)
+
+
+def _compare_spectra(o, g, min_count=1000):
+    so, sigo, no = o.spectrum()
+    sg, sigg, ng = g.spectrum()
+    sel = (no >= min_count) & (so > 0)
+    assert np.array_equal(ng[sel], no[sel]) or np.max(np.abs(ng[sel] - no[sel])) <= 3
+    rel = np.abs(sg[sel] / so[sel] - 1)
+    assert np.all(rel < 0.01), rel.max()
+    assert np.all(np.abs(sg[sel] - so[sel]) < 3 * sigo[sel] + 1e-300)
+    return sel.sum(), rel.max() if sel.any() else 0.0
+
+
+def _compare_stats(o, g, rel=1e-6):
+    so, sg = o.stats(), g.stats()
+    for kname in ("n_primary",):
+        assert so[kname] == sg[kname]
+    for kname in ("n_spawned", "n_recorded", "n_steps_total", "n_verlet_iters", "n_horizon", "n_roulette_killed"):
+        assert abs(so[kname] - sg[kname]) <= max(3, 2e-4 * so[kname]), (kname, so[kname], sg[kname])
+    for kname in ("sum_w_emit", "sum_wE_emit"):
+        assert sg[kname] == pytest.approx(so[kname], rel=1e-10)
+    for kname in ("sum_w_rec", "sum_wE_rec", "sum_w_absorbed"):
+        assert sg[kname] == pytest.approx(so[kname], rel=rel), kname
+    assert sg["n_maxstep"] == so["n_maxstep"] and sg["n_bad_scatter"] == so["n_bad_scatter"]
+
+
+def test_config0_thin_sphere(gm):
+    """BASELINE configs[0]: flat space, no scattering, N_s = 1e5."""
+    p, prim = wl.config0()
+    o, g = _pair(gm, p, prim)
+    o.run(); g.run()
+    _compare_stats(o, g)
+    nb, worst = _compare_spectra(o, g, min_count=200)
+    assert nb >= 20
+    A_o, Q_o, W_o, n_o = o.tally()
+    A_g, Q_g, W_g, n_g = g.tally()
+    assert np.array_equal(n_o, n_g)                       # every superphoton lands in the same bin
+    m = A_o > 0
+    assert np.max(_relerr(A_o[m], A_g[m])) < 1e-8
+    assert np.max(_relerr(Q_o[m], Q_g[m])) < 1e-8
+    ids = np.arange(0, g.n_primaries, 37)
+    _compare_traces(o, g, ids, fork_budget=1e-3)
+
+
+def test_scattering_off_reproduces_config0_path_bitwise(gm):
+    """DESIGN.md O7 pin: scattering_on = 0 and nsc_max = 0 give identical tallies on the GPU."""
+    p, prim = wl.config0(Ns=2e4)
+    g1 = gm.GPUMonty(p); g1.set_grid(prim); g1.prepare(); g1.run()
+    p2 = dict(p); p2.update(scattering_on=1, nsc_max=0, bias0=1.0)
+    g2 = gm.GPUMonty(p2); g2.set_grid(prim); g2.prepare(); g2.run()
+    for a, b in zip(g1.tally(), g2.tally()):
+        assert np.array_equal(a, b) or np.max(_relerr(a, b)) < 1e-13   # atomics: summation order
+
+
+def test_config1_scattering_sphere_small(gm):
+    """configs[1] at N_s = 5e4 (the oracle finishes in seconds): histories and spectrum."""
+    p, prim = wl.config1(Ns=5e4)
+    o, g = _pair(gm, p, prim)
+    o.run(); g.run()
+    so, sg = o.stats(), g.stats()
+    assert sg["n_spawned"] > 5e3
+    _compare_stats(o, g, rel=2e-3)
+    _compare_spectra(o, g, min_count=1000)
+    ids = np.arange(0, g.n_primaries, 23)
+    _compare_traces(o, g, ids, fork_budget=2e-3)
+    # weight bookkeeping on the GPU
+    out = (sg["sum_w_rec"] + sg["sum_w_horizon"] + sg["sum_w_roulette_killed"] - sg["sum_w_roulette_gain"] +
+           sg["sum_w_outofrange"] + sg["sum_w_maxstep"] + sg["sum_w_absorbed"] + sg["sum_w_bad"])
+    assert out == pytest.approx(sg["sum_w_emit"], rel=1e-9)
+
+
+def test_config2_torus_small(gm):
+    """configs[2] recipe on the full 256x256 grid at N_s = 2e4 (Kerr, R-beta electrons, biased scattering)."""
+    p, prim = wl.config2(Ns=2e4)
+    o, g = _pair(gm, p, prim)
+    o.run(); g.run()
+    sg = g.stats()
+    assert sg["n_spawned"] > 2 * sg["n_primary"] and sg["n_horizon"] > 0
+    _compare_stats(o, g, rel=5e-3)
+    _compare_spectra(o, g, min_count=1000)
+    ids = np.arange(0, g.n_primaries, 11)
+    _compare_traces(o, g, ids, fork_budget=5e-3)
+
+
+def test_config3_3d_small(gm):
+    """configs[3] recipe on a reduced 48x32x32 grid (trilinear gather, periodic x3)."""
+    p, prim = wl.config3(Ns=1e4, n1=48, n2=32, n3=32)
+    o, g = _pair(gm, p, prim)
+    assert np.array_equal(o.zone_counts(), g.zone_counts())
+    o.run(); g.run()
+    _compare_stats(o, g, rel=5e-3)
+    ids = np.arange(0, g.n_primaries, 7)
+    _compare_traces(o, g, ids, fork_budget=5e-3)
+
+
+def test_config4_analog_scattering_small(gm):
+    """configs[4]: density x1e3, analog scattering (b = 1): parents die at every event."""
+    p, prim = wl.config4(Ns=5e3)
+    o, g = _pair(gm, p, prim)
+    o.run(); g.run()
+    sg = g.stats()
+    assert sg["n_analog_killed"] > 0
+    _compare_stats(o, g, rel=5e-3)
+    ids = np.arange(0, g.n_primaries, 5)
+    _compare_traces(o, g, ids, fork_budget=5e-3)
+
+
+def test_batching_and_queue_overflow_recovery(gm):
+    """S13: id-range batches give the same tally as one batch; a queue that is too small makes the driver
+    shrink the batch and redo it (nothing dropped), never a silent loss."""
+    p, prim = wl.config1(Ns=3e4)
+    g = gm.GPUMonty(p); g.set_grid(prim); n = g.prepare(); g.run()
+    ref = g.tally(); ref_stats = g.stats()
+    g2 = gm.GPUMonty(p); g2.set_grid(prim); g2.prepare()
+    g2.set_batch(4096, 3000)          # children of 4096 primaries (~3-4x) cannot fit 3000 records
+    g2.run(0, n // 3); g2.run(n // 3, n - n // 3)
+    got = g2.tally(); st = g2.stats()
+    assert np.array_equal(ref[3], got[3])
+    assert np.max(_relerr(ref[0], got[0], floor=1e-300)) < 1e-12
+    assert st["n_spawned"] == ref_stats["n_spawned"] and st["n_primary"] == ref_stats["n_primary"]
+
+
+def test_empty_and_degenerate_inputs(gm):
+    p, prim = wl.config0(Ns=1e3)
+    g = gm.GPUMonty(p); g.set_grid(prim); n = g.prepare()
+    g.run(0, 0)
+    assert g.stats()["n_primary"] == 0
+    with pytest.raises(gm.GmError):
+        g.run(0, n + 1)
+    # a grid with no emitting zone: zero primaries, empty spectrum
+    cold = prim.copy(); cold[..., 5:8] = 0.0
+    g3 = gm.GPUMonty(p); g3.set_grid(cold)
+    assert g3.prepare() == 0
+    g3.run()
+    assert g3.spectrum()[0].sum() == 0.0
+    bad = prim.copy(); bad[3, 2, 0, 1] = np.nan
+    g4 = gm.GPUMonty(p); g4.set_grid(bad)
+    with pytest.raises(gm.GmError):
+        g4.prepare()
+    q = dict(p); q["nu_min"] = q["nu_max"]
+    with pytest.raises(gm.GmError):
+        gm.GPUMonty(q)
+
+
+def test_device_grid_input_and_stream(gm):
+    """The grid may be a CUDA tensor and the work may run on a non-default torch stream."""
+    import torch
+    p, prim = wl.config0(Ns=2e4)
+    g1 = gm.GPUMonty(p); g1.set_grid(prim); g1.prepare(); g1.run()
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        t = torch.from_numpy(prim).cuda()
+        g2 = gm.GPUMonty(p); g2.set_grid(t); g2.prepare(); g2.run()
+    assert np.array_equal(g1.tally()[3], g2.tally()[3])
