@@ -1,0 +1,272 @@
+#!/usr/bin/env python
+"""Benchmark of the superphoton transport hot path (one JSON line on stdout; contract in DESIGN.md "Measurement").
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--ns NS] [--impl reference]
+
+A step is one pass of the whole path of SURVEY.md 8(a) over one synthetic workload: device tables (S0), weights,
+zone counts and prefix sum (S1-S4), emission (S5), tracking with absorption and scattering (S6-S10, S12), Compton
+events (S11) in id-range batches (S13), and the spectrum scaling.  `value` is superphotons/s (emitted + scattered,
+the paper's own count) with the fluid grid already resident in HBM; `e2e` is the same through the
+C-ABI with HOST buffers (pinned grid in, spectrum out) inside the timed region.
+
+Default workload: BASELINE.json configs[2] (2-D Kerr torus, N_s = 1e7) -- the single-GPU stand-in for the GRMHD
+run on which the paper quotes its superphotons/s; `--config` selects another.
+`--impl reference` times the CPU oracle (as it stands) on a bounded id sub-range of the same workload.
+Under torchrun (N > 1) each rank runs the same workload with its own Philox seed (weak scaling: histories are
+independent, no data-path collective); the tallies are summed once at the end.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2602_13198_b200 import workloads as wl  # noqa: E402
+from paper_2602_13198_b200.shard import rank_seed, reduce_tally  # noqa: E402
+
+METRIC = "superphotons/s tracked (incl. scattering)"
+UNIT = "superphotons/s"
+# algorithmic FP64 flop per geodesic step of the tracker (dadd + dmul + 2 dfma thread
+# instructions per committed step, counted once with ncu on each workload class and then frozen)
+FLOP_PER_STEP = {"flat": 1.30e3, "kerr": 2.20e3}
+WORKLOAD_NAMES = {0: "cfg0 thin synchrotron sphere 32x16, Ns=1e5", 1: "cfg1 scattering sphere 32x16, Ns=1e6",
+                  2: "cfg2 Kerr FM torus 256x256, Ns=1e7", 3: "cfg3 3-D perturbed torus 192x128x128, Ns=1e7",
+                  4: "cfg4 Kerr torus x1e3 density (analog scattering), Ns=1e6"}
+
+
+def make_workload(cfg: int, ns: float | None, seed: int):
+    kw = {"seed": seed}
+    if ns:
+        kw["Ns"] = ns
+    p, prim = wl.CONFIGS[cfg](**kw)
+    return p, prim
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons sampled DURING the timed region (profiling recipe)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_sample(p, prim, n_sample_primaries: int, threads: int = 0):
+    """Time the CPU oracle (as it stands) on the first n primaries + all their descendants."""
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    from oracle_binding import Oracle
+    o = Oracle(p, prim)
+    t0 = time.perf_counter()
+    n = o.prepare()
+    t1 = time.perf_counter()
+    m = min(n, n_sample_primaries)
+    used = o.run(0, m, threads)
+    t2 = time.perf_counter()
+    s = o.stats()
+    tracked = s["n_primary"] + s["n_spawned"]
+    return {"tracked": tracked, "run_s": t2 - t1, "prepare_s": t1 - t0, "cores": used, "n_sample": m,
+            "steps": s["n_steps_total"]}
+
+
+def run_reference(args, rank, world):
+    if rank != 0:
+        return
+    p, prim = make_workload(args.config, args.ns, 1)
+    # bounded sample per step: sized from a quick probe so that K+W steps end within a few minutes
+    probe = oracle_sample(p, prim, 2000)
+    rate = probe["tracked"] / max(probe["run_s"], 1e-6)
+    per_primary = probe["tracked"] / max(probe["n_sample"], 1)
+    target_s = min(20.0, 150.0 / max(1, args.steps + args.warmup))
+    n_sample = int(max(500, rate * target_s / per_primary))
+    times, tracked = [], 0
+    for it in range(args.warmup + args.steps):
+        r = oracle_sample(p, prim, n_sample)
+        if it >= args.warmup:
+            times.append(r["run_s"] + r["prepare_s"]); tracked = r["tracked"]; cores = r["cores"]
+    ms = 1e3 * float(np.mean(times))
+    value = tracked / (ms * 1e-3)
+    sample = f"first {n_sample} primaries of {WORKLOAD_NAMES[args.config]} + all descendants per step (oracle prepare included)"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": 0, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic", "config": {"workload": WORKLOAD_NAMES[args.config], "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=2, choices=sorted(wl.CONFIGS))
+    ap.add_argument("--ns", type=float, default=None, help="override N_s of the config")
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_2602_13198_b200 import binding as gm
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; this path has no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    stream = torch.cuda.current_stream()
+
+    p, prim = make_workload(args.config, args.ns, rank_seed(1, rank))
+    g = gm.GPUMonty(p)
+    host_grid = torch.from_numpy(prim).pin_memory()
+    dev_grid = host_grid.cuda()
+    flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.float32, device="cuda")   # > 126 MB L2
+    nb = p["n_th"] * p["n_nu"]
+    d_spec = torch.zeros(2, nb, dtype=torch.float64, device="cuda")
+
+    def step(e2e: bool):
+        g.build_tables(stream)
+        g.set_grid(host_grid if e2e else dev_grid, stream)
+        g.prepare(stream)
+        g.run(stream=stream)
+        if e2e:
+            return g.spectrum()
+        g.spectrum_device(d_spec[0], d_spec[1], stream)
+        return None
+
+    def timed(e2e: bool, nsteps: int):
+        ms = []
+        for _ in range(nsteps):
+            flush.fill_(1.0)                                  # L2 flush between timed iterations
+            if world > 1:
+                dist.barrier()
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            step(e2e)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            ms.append(e0.elapsed_time(e1))
+        return ms
+
+    for _ in range(args.warmup):
+        step(False)
+    torch.cuda.synchronize()
+    g.timing(True)
+    clocks = ClockSampler(local)
+    clocks.start()
+    ms_dev = timed(False, args.steps)
+    clk = clocks.stop()
+    tm = g.timing(False)
+    st = g.stats()
+    tracked = st["n_primary"] + st["n_spawned"]
+    ms_e2e = timed(True, args.steps)
+
+    t_dev = torch.tensor([float(np.mean(ms_dev)), float(np.mean(ms_e2e))], device="cuda", dtype=torch.float64)
+    cnt = torch.tensor([float(tracked)], device="cuda", dtype=torch.float64)
+    if world > 1:
+        dist.all_reduce(t_dev, op=dist.ReduceOp.MAX)
+        dist.all_reduce(cnt, op=dist.ReduceOp.SUM)
+        reduce_tally([torch.from_numpy(a).cuda() for a in g.tally()], dist)   # combined spectrum of the N runs
+    ms_step, ms_step_e2e = float(t_dev[0]), float(t_dev[1])
+    total = float(cnt[0])
+
+    if rank == 0:
+        value = total / (ms_step * 1e-3)
+        kind = "kerr" if p["metric_kind"] == 1 else "flat"
+        n_track_launches = max(1, tm["track"][1])
+        flops = st["n_steps_total"] * FLOP_PER_STEP[kind]           # this rank, last timed step
+        track_ms_per_step = tm["track"][0] / args.steps
+        peak_meas, _ = gm.fp64_peak()
+        achieved = flops / (track_ms_per_step * 1e-3) / 1e12
+        peak = peak_meas / 1e12
+        launches = sum(v[1] for v in tm.values()) // max(1, args.steps)
+        out = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic",
+            "config": {"workload": WORKLOAD_NAMES[args.config] + (f" (Ns overridden: {args.ns:g})" if args.ns else ""),
+                       "superphotons_per_step_per_gpu": tracked, "primaries": st["n_primary"], "spawned": st["n_spawned"],
+                       "geodesic_steps": st["n_steps_total"], "l2": "flushed between timed steps (256 MB write)",
+                       "multi_gpu": "one independent seeded run per rank, tallies summed once" if world > 1 else "single GPU"},
+            "e2e": {"value": total / (ms_step_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(prim.nbytes),
+                    "d2h_bytes_per_step": int(nb * 8 * 3), "ms_per_step": ms_step_e2e},
+            "gpu_launches": int(launches),
+            "clocks": clk,
+            "roofline": {"bound": "alu", "kernel": "track_kernel", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                         "frac": achieved / peak, "traffic": None,
+                         "peak_source": "DFMA-chain microbenchmark run in this process (gm_fp64_peak); nominal 2*64*148*1.965 GHz = 37.2",
+                         "flop_per_step": FLOP_PER_STEP[kind], "track_ms_per_step": track_ms_per_step,
+                         "track_launches_per_step": n_track_launches // max(1, args.steps),
+                         "track_share_of_step": track_ms_per_step / ms_step,
+                         "kernel_ms_per_step": {k: v[0] / args.steps for k, v in tm.items()}},
+        }
+        if not args.no_cpu_baseline and world == 1:
+            pr = oracle_sample(p, prim, 20000)        # probe (also pays the one-off oracle table build)
+            pr = oracle_sample(p, prim, 20000)
+            rate = pr["tracked"] / max(pr["run_s"], 1e-6)
+            n_sample = int(max(20000, rate * 15.0 / (pr["tracked"] / max(1, pr["n_sample"]))))
+            r = oracle_sample(p, prim, n_sample)
+            out["cpu_baseline"] = {"value": r["tracked"] / r["run_s"], "unit": UNIT, "cores": r["cores"], "kind": "oracle",
+                                   "sample": f"first {r['n_sample']} primaries + descendants ({r['tracked']} superphotons, "
+                                             f"{r['run_s']:.1f} s, oracle prepare {r['prepare_s']:.1f} s not counted)"}
+        print(json.dumps(out))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -124,6 +124,9 @@ typedef struct gm_ctx gm_ctx; /* opaque; owned by the library */
  * gm_last_error(NULL)). */
 int gm_create(gm_ctx** out, const gm_params* p);
 void gm_destroy(gm_ctx* ctx);
+/* (Re)build the parameter-free device tables K2, F and (if scattering_on) sigma_h on `cuda_stream`
+ * (PAPER.md:166, 188).  gm_create calls it once; a benchmark may call it per step. */
+int gm_build_tables(gm_ctx* ctx, void* cuda_stream);
 /* Message of the last failing call on ctx (or of the last failing gm_create when ctx == NULL). */
 const char* gm_last_error(const gm_ctx* ctx);
 
@@ -152,6 +155,8 @@ int gm_set_batch(gm_ctx* ctx, int64_t batch_primaries, int64_t queue_records);
 /* nu L_nu [erg/s], its Monte Carlo sigma [erg/s] and the number of superphotons per [n_th][n_nu]
  * bin (O9).  Any of the three may be NULL. */
 int gm_get_spectrum(gm_ctx* ctx, double* nuLnu, double* sigma, int64_t* nphot);
+/* Same scaling written to caller-owned DEVICE buffers [n_th][n_nu] on `cuda_stream`, no synchronisation. */
+int gm_spectrum_device(gm_ctx* ctx, double* d_nuLnu, double* d_sigma, void* cuda_stream);
 /* Raw accumulators per bin: sum wE, sum (wE)^2, sum w, count.  Any may be NULL. */
 int gm_get_tally(gm_ctx* ctx, double* A, double* Q, double* W, int64_t* n);
 int gm_get_stats(gm_ctx* ctx, gm_stats* out);
@@ -164,6 +169,13 @@ int gm_trace(gm_ctx* ctx, const int64_t* ids, int n, gm_trace_rec* out);
 /* Evaluate one device function of the path on n inputs (GM_EVAL_*): `in` and `out` are HOST arrays
  * of n rows with the row lengths listed at GM_EVAL_*. */
 int gm_eval(gm_ctx* ctx, int what, const double* in, int n, double* out);
+
+/* Per-kernel device times.  Returns, per category GM_T_*, the summed CUDA-event duration [ms] and the
+ * number of kernel launches since the previous gm_timing call, then clears the record and switches
+ * recording on (enable != 0) or off.  Synchronises the device.  ms_out / launches_out: [GM_T_COUNT]. */
+enum { GM_T_TABLES = 0, GM_T_PREPARE = 1, GM_T_EMIT = 2, GM_T_TRACK = 3, GM_T_COMPTON = 4, GM_T_SPECTRUM = 5,
+       GM_T_COUNT = 6 };
+int gm_timing(gm_ctx* ctx, int enable, double* ms_out, int64_t* launches_out);
 
 /* sizeof(gm_params), sizeof(gm_stats), sizeof(gm_trace_rec), sizeof(gm_emit_rec): lets a binding check its
  * struct layouts against the library's. */

@@ -23,7 +23,7 @@ FATE_ALIVE, FATE_RECORDED, FATE_HORIZON, FATE_ROULETTE, FATE_MAXSTEP, FATE_OUTOF
 
 EXPORTS = ["gm_create", "gm_destroy", "gm_last_error", "gm_set_grid", "gm_prepare", "gm_get_zone_counts",
            "gm_get_table", "gm_run", "gm_set_batch", "gm_get_spectrum", "gm_get_tally", "gm_get_stats",
-           "gm_reset_tally", "gm_emit", "gm_trace", "gm_eval", "gm_fp64_peak"]
+           "gm_reset_tally", "gm_emit", "gm_trace", "gm_eval", "gm_fp64_peak", "gm_build_tables", "gm_timing", "gm_spectrum_device"]
 
 
 class GmParams(C.Structure):
@@ -102,6 +102,9 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
     L.gm_eval.argtypes = [vp, C.c_int, vp, C.c_int, vp]
     L.gm_fp64_peak.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double)]
     L.gm_abi_sizes.argtypes = [C.POINTER(C.c_int)]
+    L.gm_build_tables.argtypes = [vp, vp]
+    L.gm_spectrum_device.argtypes = [vp, vp, vp, vp]
+    L.gm_timing.argtypes = [vp, C.c_int, vp, vp]
     L.gm_abi_sizes.restype = None
     _lib = L
     return L
@@ -202,6 +205,16 @@ class GPUMonty:
             n = self.n_primaries - first
         self._ck(self.L.gm_run(self.h, int(first), int(n), _stream_ptr(stream)))
 
+    def build_tables(self, stream=None):
+        self._ck(self.L.gm_build_tables(self.h, _stream_ptr(stream)))
+
+    def timing(self, enable=True):
+        """{category: (ms, launches)} since the previous call; switches per-kernel event timing on/off."""
+        ms, nl = np.zeros(6), np.zeros(6, dtype=np.int64)
+        self._ck(self.L.gm_timing(self.h, int(enable), _np_ptr(ms), _np_ptr(nl)))
+        names = ("tables", "prepare", "emit", "track", "compton", "spectrum")
+        return {n: (float(ms[i]), int(nl[i])) for i, n in enumerate(names)}
+
     def reset_tally(self):
         self._ck(self.L.gm_reset_tally(self.h))
 
@@ -223,6 +236,11 @@ class GPUMonty:
         a, s, n = np.zeros(nb), np.zeros(nb), np.zeros(nb, dtype=np.int64)
         self._ck(self.L.gm_get_spectrum(self.h, _np_ptr(a), _np_ptr(s), _np_ptr(n)))
         return a.reshape(self.shape), s.reshape(self.shape), n.reshape(self.shape)
+
+    def spectrum_device(self, nuLnu, sigma, stream=None):
+        """nu L_nu and sigma into caller-owned CUDA tensors (fp64, n_th*n_nu elements), asynchronously."""
+        self._ck(self.L.gm_spectrum_device(self.h, C.c_void_p(nuLnu.data_ptr()), C.c_void_p(sigma.data_ptr()),
+                                           _stream_ptr(stream)))
 
     def tally(self):
         nb = self.shape[0] * self.shape[1]

@@ -31,7 +31,30 @@ struct gm_ctx {
   bool have_grid = false, prepared = false;
   long long n_primaries = 0;
   std::string err;
+  // per-kernel timing: event pairs recorded around every launch (categories GM_T_*)
+  std::vector<cudaEvent_t> ev_pool;
+  std::vector<int> ev_cat;       // category of pair i (events 2i, 2i+1)
+  size_t ev_used = 0;
+  bool timing = false;
 };
+
+static void t_begin(gm_ctx* c, int cat, cudaStream_t st) {
+  if (!c->timing) return;
+  if (c->ev_used + 2 > c->ev_pool.size()) {
+    if (c->ev_pool.size() >= 16384) return;
+    for (int i = 0; i < 256; i++) { cudaEvent_t e; cudaEventCreate(&e); c->ev_pool.push_back(e); }
+  }
+  c->ev_cat.push_back(cat);
+  cudaEventRecord(c->ev_pool[c->ev_used], st);
+  c->ev_used += 1;
+}
+static void t_end(gm_ctx* c, cudaStream_t st) {
+  if (!c->timing || (c->ev_used & 1) == 0) return;
+  cudaEventRecord(c->ev_pool[c->ev_used], st);
+  c->ev_used += 1;
+}
+#define TIMED(cat, st, call) do { t_begin(ctx, cat, st); cudaError_t e__ = (call); t_end(ctx, st); \
+    if (e__ != cudaSuccess) return fail(ctx, GM_ERR_CUDA, "%s: %s", #call, cudaGetErrorString(e__)); } while (0)
 
 static std::string g_create_err;
 
@@ -65,6 +88,8 @@ static void free_all(gm_ctx* c) {
   cudaFree(c->Z.blocksum); cudaFree(c->Z.bad);
   cudaFree(c->tally.A); cudaFree(c->tally_snap.A);
   cudaFree(c->d_stats); cudaFree(c->d_stats_snap); cudaFree(c->d_spec); cudaFree(c->d_counters);
+  for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
+  c->ev_pool.clear();
 }
 
 static bool finite_pos(double v) { return std::isfinite(v) && v > 0.0; }
@@ -198,9 +223,7 @@ int gm_create(gm_ctx** out, const gm_params* p) {
   ctx->tally_snap.n = (unsigned long long*)(ctx->tally_snap.A + 3 * nb);
   fill_dev_params(ctx);
   // parameter-free tables (S0)
-  cudaError_t te = build_K2_table(ctx->d_lnK2, 0);
-  if (te == cudaSuccess) te = build_F_table(ctx->d_lnF, 0);
-  if (te == cudaSuccess && p->scattering_on) te = build_sigh_table(ctx->d_lnSigH, 0);
+  cudaError_t te = gm_build_tables(ctx, nullptr) == GM_OK ? cudaSuccess : cudaErrorUnknown;
   if (te == cudaSuccess) te = cudaMemset(ctx->tally.A, 0, (size_t)nb * 4 * sizeof(double));
   if (te == cudaSuccess) te = cudaMemset(ctx->d_stats, 0, sizeof(DevStats));
   if (te == cudaSuccess) te = cudaDeviceSynchronize();
@@ -210,6 +233,15 @@ int gm_create(gm_ctx** out, const gm_params* p) {
     return fail(nullptr, GM_ERR_CUDA, "table build failed: %s", m.c_str());
   }
   *out = ctx;
+  return GM_OK;
+}
+
+int gm_build_tables(gm_ctx* ctx, void* cuda_stream) {
+  if (!ctx) return GM_ERR_PARAM;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  TIMED(GM_T_TABLES, st, build_K2_table(ctx->d_lnK2, st));
+  TIMED(GM_T_TABLES, st, build_F_table(ctx->d_lnF, st));
+  if (ctx->p.scattering_on) TIMED(GM_T_TABLES, st, build_sigh_table(ctx->d_lnSigH, st));
   return GM_OK;
 }
 
@@ -248,7 +280,7 @@ int gm_prepare(gm_ctx* ctx, void* cuda_stream, int64_t* n_primaries_out) {
   for (int k = 0; k <= NW; k++) nu_nodes[k] = ctx->p.nu_min * std::exp(k * Dl);
   CK(cudaMemcpyAsync(ctx->Z.nu_nodes, nu_nodes, sizeof(nu_nodes), cudaMemcpyHostToDevice, st));
   CK(cudaMemsetAsync(ctx->Z.bad, 0, sizeof(int), st));
-  CK(launch_prepare(ctx->P, ctx->Z, ctx->d_lnw, ctx->nz, st));
+  TIMED(GM_T_PREPARE, st, launch_prepare(ctx->P, ctx->Z, ctx->d_lnw, ctx->nz, st));
   long long total = 0;
   int bad = 0;
   CK(cudaMemcpyAsync(&total, ctx->Z.offset + ctx->nz, sizeof(long long), cudaMemcpyDeviceToHost, st));
@@ -327,7 +359,7 @@ static int run_batch(gm_ctx* ctx, long long first, int n, const long long* d_ids
                      Tally tally, DevStats* stats, cudaStream_t st, int* max_queue) {
   int* cnt = ctx->d_counters;       // [0] primaries, [1] work counter, [2 + layer] queue filled by that layer
   CK(cudaMemsetAsync(cnt, 0, 64 * sizeof(int), st));
-  CK(launch_emit(ctx->P, ctx->Z, ctx->nz, first, n, d_ids, ctx->d_prim_ph, cnt + 0, stats, nullptr, with_root, st));
+  TIMED(GM_T_EMIT, st, launch_emit(ctx->P, ctx->Z, ctx->nz, first, n, d_ids, ctx->d_prim_ph, cnt + 0, stats, nullptr, with_root, st));
   const int qcap = (int)ctx->queue_records;
   const Photon* in = ctx->d_prim_ph;
   const int* in_count = cnt + 0;
@@ -335,9 +367,9 @@ static int run_batch(gm_ctx* ctx, long long first, int n, const long long* d_ids
   const int layers = ctx->p.scattering_on ? ctx->p.nsc_max : 0;
   for (int layer = 0; layer <= layers; layer++) {
     Queue out{(layer & 1) ? ctx->d_qB : ctx->d_qA, cnt + 2 + layer, qcap};
-    CK(launch_track(ctx->P, in, in_count, in_cap, cnt + 1, out, tally, stats, trace, ctx->n_sm, st));
+    TIMED(GM_T_TRACK, st, launch_track(ctx->P, in, in_count, in_cap, cnt + 1, out, tally, stats, trace, ctx->n_sm, st));
     if (layer == layers) break;
-    CK(launch_compton(ctx->P, out, stats, trace, ctx->n_sm, st));
+    TIMED(GM_T_COMPTON, st, launch_compton(ctx->P, out, stats, trace, ctx->n_sm, st));
     in = out.buf; in_count = out.count; in_cap = qcap;
   }
   int h_counts[64];
@@ -402,11 +434,18 @@ int gm_get_tally(gm_ctx* ctx, double* A, double* Q, double* W, int64_t* n) {
 int gm_get_spectrum(gm_ctx* ctx, double* nuLnu, double* sigma, int64_t* nphot) {
   if (!ctx) return GM_ERR_PARAM;
   const size_t nb = (size_t)ctx->p.n_th * ctx->p.n_nu;
-  CK(launch_spectrum(ctx->P, ctx->tally, ctx->d_spec, ctx->d_spec + nb, 0));
+  TIMED(GM_T_SPECTRUM, 0, launch_spectrum(ctx->P, ctx->tally, ctx->d_spec, ctx->d_spec + nb, 0));
   CK(cudaDeviceSynchronize());
   if (nuLnu) CK(cudaMemcpy(nuLnu, ctx->d_spec, nb * 8, cudaMemcpyDeviceToHost));
   if (sigma) CK(cudaMemcpy(sigma, ctx->d_spec + nb, nb * 8, cudaMemcpyDeviceToHost));
   if (nphot) CK(cudaMemcpy(nphot, ctx->tally.n, nb * 8, cudaMemcpyDeviceToHost));
+  return GM_OK;
+}
+
+int gm_spectrum_device(gm_ctx* ctx, double* d_nuLnu, double* d_sigma, void* cuda_stream) {
+  if (!ctx || !d_nuLnu || !d_sigma) return GM_ERR_PARAM;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  TIMED(GM_T_SPECTRUM, st, launch_spectrum(ctx->P, ctx->tally, d_nuLnu, d_sigma, st));
   return GM_OK;
 }
 
@@ -493,6 +532,27 @@ int gm_eval(gm_ctx* ctx, int what, const double* in, int n, double* out) {
   if (e == cudaSuccess) e = cudaMemcpy(out, d_out, (size_t)n * nout[what] * sizeof(double), cudaMemcpyDeviceToHost);
   cudaFree(d_in); cudaFree(d_out);
   if (e != cudaSuccess) return fail(ctx, GM_ERR_CUDA, "gm_eval: %s", cudaGetErrorString(e));
+  return GM_OK;
+}
+
+int gm_timing(gm_ctx* ctx, int enable, double* ms_out, int64_t* launches_out) {
+  if (!ctx) return GM_ERR_PARAM;
+  CK(cudaDeviceSynchronize());
+  double ms[GM_T_COUNT] = {0};
+  int64_t nl[GM_T_COUNT] = {0};
+  for (size_t i = 0; i + 1 < ctx->ev_used; i += 2) {
+    float t = 0.f;
+    if (cudaEventElapsedTime(&t, ctx->ev_pool[i], ctx->ev_pool[i + 1]) == cudaSuccess) {
+      int c = ctx->ev_cat[i / 2];
+      ms[c] += t; nl[c] += 1;
+    }
+  }
+  // kernels per launch wrapper: tables 1, prepare 7, others 1
+  nl[GM_T_PREPARE] *= 7;
+  if (ms_out) for (int c = 0; c < GM_T_COUNT; c++) ms_out[c] = ms[c];
+  if (launches_out) for (int c = 0; c < GM_T_COUNT; c++) launches_out[c] = nl[c];
+  ctx->ev_used = 0; ctx->ev_cat.clear();
+  ctx->timing = enable != 0;
   return GM_OK;
 }
 
