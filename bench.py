@@ -227,7 +227,8 @@ def main():
         value = total / (ms_step * 1e-3)
         kind = "kerr" if p["metric_kind"] == 1 else "flat"
         n_track_launches = max(1, tm["track"][1])
-        flops = st["n_steps_total"] * FLOP_PER_STEP[kind]           # this rank, last timed step
+        steps_track = st["n_steps_total"] - st["n_steps_free"]      # steps taken inside track_kernel (this rank, last timed step)
+        flops = steps_track * FLOP_PER_STEP[kind]
         track_ms_per_step = tm["track"][0] / args.steps
         peak_meas, _ = gm.fp64_peak()
         achieved = flops / (track_ms_per_step * 1e-3) / 1e12
@@ -239,7 +240,7 @@ def main():
             "data": "synthetic",
             "config": {"workload": WORKLOAD_NAMES[args.config] + (f" (Ns overridden: {args.ns:g})" if args.ns else ""),
                        "superphotons_per_step_per_gpu": tracked, "primaries": st["n_primary"], "spawned": st["n_spawned"],
-                       "geodesic_steps": st["n_steps_total"], "l2": "flushed between timed steps (256 MB write)",
+                       "geodesic_steps": st["n_steps_total"], "geodesic_steps_free_flight": st["n_steps_free"], "l2": "flushed between timed steps (256 MB write)",
                        "multi_gpu": "one independent seeded run per rank, tallies summed once" if world > 1 else "single GPU"},
             "e2e": {"value": total / (ms_step_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(prim.nbytes),
                     "d2h_bytes_per_step": int(nb * 8 * 3), "ms_per_step": ms_step_e2e},

@@ -75,7 +75,9 @@ typedef struct gm_params {
 typedef struct gm_stats {
   int64_t n_primary, n_spawned, n_recorded, n_horizon, n_roulette_killed, n_roulette_survived,
       n_maxstep, n_outofrange, n_steps_total, n_verlet_iters, n_verlet_capped, n_bad_scatter,
-      n_analog_killed;
+      n_analog_killed,
+      n_steps_free,   /* of n_steps_total: steps taken in free flight beyond the grid (escape kernel) */
+      n_reentered;    /* superphotons that came back into the grid from free flight                  */
   double sum_w_emit, sum_w_rec, sum_w_horizon, sum_w_roulette_killed, sum_w_roulette_gain,
       sum_w_outofrange, sum_w_maxstep, sum_w_absorbed, sum_wE_emit, sum_wE_rec, sum_w_bad;
 } gm_stats;
@@ -174,7 +176,7 @@ int gm_eval(gm_ctx* ctx, int what, const double* in, int n, double* out);
  * number of kernel launches since the previous gm_timing call, then clears the record and switches
  * recording on (enable != 0) or off.  Synchronises the device.  ms_out / launches_out: [GM_T_COUNT]. */
 enum { GM_T_TABLES = 0, GM_T_PREPARE = 1, GM_T_EMIT = 2, GM_T_TRACK = 3, GM_T_COMPTON = 4, GM_T_SPECTRUM = 5,
-       GM_T_COUNT = 6 };
+       GM_T_ESCAPE = 6, GM_T_COUNT = 7 };
 int gm_timing(gm_ctx* ctx, int enable, double* ms_out, int64_t* launches_out);
 
 /* sizeof(gm_params), sizeof(gm_stats), sizeof(gm_trace_rec), sizeof(gm_emit_rec): lets a binding check its

@@ -49,7 +49,7 @@ class GmStats(C.Structure):
     _fields_ = [(n, C.c_int64) for n in (
         "n_primary", "n_spawned", "n_recorded", "n_horizon", "n_roulette_killed", "n_roulette_survived",
         "n_maxstep", "n_outofrange", "n_steps_total", "n_verlet_iters", "n_verlet_capped", "n_bad_scatter",
-        "n_analog_killed")] + [(n, C.c_double) for n in (
+        "n_analog_killed", "n_steps_free", "n_reentered")] + [(n, C.c_double) for n in (
         "sum_w_emit", "sum_w_rec", "sum_w_horizon", "sum_w_roulette_killed", "sum_w_roulette_gain",
         "sum_w_outofrange", "sum_w_maxstep", "sum_w_absorbed", "sum_wE_emit", "sum_wE_rec", "sum_w_bad")]
 
@@ -210,9 +210,9 @@ class GPUMonty:
 
     def timing(self, enable=True):
         """{category: (ms, launches)} since the previous call; switches per-kernel event timing on/off."""
-        ms, nl = np.zeros(6), np.zeros(6, dtype=np.int64)
+        ms, nl = np.zeros(7), np.zeros(7, dtype=np.int64)
         self._ck(self.L.gm_timing(self.h, int(enable), _np_ptr(ms), _np_ptr(nl)))
-        names = ("tables", "prepare", "emit", "track", "compton", "spectrum")
+        names = ("tables", "prepare", "emit", "track", "compton", "spectrum", "escape")
         return {n: (float(ms[i]), int(nl[i])) for i, n in enumerate(names)}
 
     def reset_tally(self):

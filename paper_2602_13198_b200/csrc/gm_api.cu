@@ -25,7 +25,8 @@ struct gm_ctx {
   DevStats *d_stats = nullptr, *d_stats_snap = nullptr;
   double *d_spec = nullptr;          // [2][nb]
   int* d_counters = nullptr;         // [0] primaries count, [1] queue A count, [2] queue B count, [3] work counter
-  Photon *d_prim_ph = nullptr, *d_qA = nullptr, *d_qB = nullptr;
+  Photon *d_prim_ph = nullptr, *d_qA = nullptr, *d_qB = nullptr, *d_esc = nullptr;
+  long long esc_records = 0;
   long long batch_primaries = 0, queue_records = 0;   // allocated sizes
   long long want_batch = 0, want_queue = 0;
   bool have_grid = false, prepared = false;
@@ -74,9 +75,9 @@ static int fail(gm_ctx* c, int code, const char* fmt, ...) {
   } while (0)
 
 static void free_run_buffers(gm_ctx* c) {
-  cudaFree(c->d_prim_ph); cudaFree(c->d_qA); cudaFree(c->d_qB);
-  c->d_prim_ph = c->d_qA = c->d_qB = nullptr;
-  c->batch_primaries = c->queue_records = 0;
+  cudaFree(c->d_prim_ph); cudaFree(c->d_qA); cudaFree(c->d_qB); cudaFree(c->d_esc);
+  c->d_prim_ph = c->d_qA = c->d_qB = c->d_esc = nullptr;
+  c->batch_primaries = c->queue_records = c->esc_records = 0;
 }
 
 static void free_all(gm_ctx* c) {
@@ -342,41 +343,60 @@ static int ensure_run_buffers(gm_ctx* ctx, long long n_ids) {
     batch = 1024;
     while (batch < n_ids) batch <<= 1;           // power of two >= n_ids: a later, larger gm_run re-allocates
   }
-  long long queue = ctx->want_queue ? ctx->want_queue : (ctx->p.scattering_on ? 4 * batch : 1);
-  if (!ctx->p.scattering_on) queue = 1;
-  // size the batch from the free device memory
-  while ((size_t)(batch + 2 * queue) * sizeof(Photon) > free_b / 2 && batch > 1024) { batch >>= 1; if (!ctx->want_queue && ctx->p.scattering_on) queue = 4 * batch; }
+  // scattered-superphoton queues: 8 records per primary by default (7-10x N_s are generated in
+  // total, spread over the scattering generations); the escape queue must hold one whole tracker input
+  const bool sc = ctx->p.scattering_on != 0;
+  // (without scattering the queue only ever holds re-entrants from free flight: none in flat space)
+  const bool kerr = ctx->p.metric_kind == 1;
+  auto queue_for = [&](long long b) { return ctx->want_queue ? ctx->want_queue : (sc ? 8 * b : (kerr ? b : 1)); };
+  long long queue = queue_for(batch);
+  // size the batch from the free device memory (at most half of it)
+  auto bytes = [&](long long b, long long q) { return (size_t)(b + 2 * q + (b > q ? b : q)) * sizeof(Photon); };
+  while (bytes(batch, queue) > free_b / 2 && batch > 1024) { batch >>= 1; queue = queue_for(batch); }
+  const long long esc = batch > queue ? batch : queue;
   CK(cudaMalloc((void**)&ctx->d_prim_ph, (size_t)batch * sizeof(Photon)));
   CK(cudaMalloc((void**)&ctx->d_qA, (size_t)queue * sizeof(Photon)));
   CK(cudaMalloc((void**)&ctx->d_qB, (size_t)queue * sizeof(Photon)));
-  ctx->batch_primaries = batch; ctx->queue_records = queue;
+  CK(cudaMalloc((void**)&ctx->d_esc, (size_t)esc * sizeof(Photon)));
+  ctx->batch_primaries = batch; ctx->queue_records = queue; ctx->esc_records = esc;
   return GM_OK;
 }
 
-// one batch: emit -> [track -> compton] per scattering generation.  Returns the largest queue
-// occupancy seen (device counters may exceed the capacity: overflow).
+// one batch: emit -> per scattering generation [track -> compton (events -> scattered superphotons) -> escape
+// (free flight of the leavers; re-entrants are appended behind the scattered superphotons)].  Returns the
+// largest queue occupancy seen (device counters may exceed the capacity: overflow).
 static int run_batch(gm_ctx* ctx, long long first, int n, const long long* d_ids, TraceBuf trace, bool with_root,
                      Tally tally, DevStats* stats, cudaStream_t st, int* max_queue) {
-  int* cnt = ctx->d_counters;       // [0] primaries, [1] work counter, [2 + layer] queue filled by that layer
-  CK(cudaMemsetAsync(cnt, 0, 64 * sizeof(int), st));
+  int* cnt = ctx->d_counters;       // [0] primaries, [1] work counter, [2] escape queue, [3 + round] queue filled by that round
+  const int NCNT = 64, MAXROUND = NCNT - 3;
+  CK(cudaMemsetAsync(cnt, 0, NCNT * sizeof(int), st));
   TIMED(GM_T_EMIT, st, launch_emit(ctx->P, ctx->Z, ctx->nz, first, n, d_ids, ctx->d_prim_ph, cnt + 0, stats, nullptr, with_root, st));
   const int qcap = (int)ctx->queue_records;
   const Photon* in = ctx->d_prim_ph;
   const int* in_count = cnt + 0;
   int in_cap = (int)ctx->batch_primaries;
   const int layers = ctx->p.scattering_on ? ctx->p.nsc_max : 0;
-  for (int layer = 0; layer <= layers; layer++) {
-    Queue out{(layer & 1) ? ctx->d_qB : ctx->d_qA, cnt + 2 + layer, qcap};
-    TIMED(GM_T_TRACK, st, launch_track(ctx->P, in, in_count, in_cap, cnt + 1, out, tally, stats, trace, ctx->n_sm, st));
-    if (layer == layers) break;
-    TIMED(GM_T_COMPTON, st, launch_compton(ctx->P, out, stats, trace, ctx->n_sm, st));
-    in = out.buf; in_count = out.count; in_cap = qcap;
+  Queue esc{ctx->d_esc, cnt + 2, (int)ctx->esc_records};
+  int h_counts[NCNT];
+  int mq = 0, round = 0;
+  for (;;) {
+    // generations 0..layers without a host round trip; afterwards only while re-entrants keep a queue non-empty
+    const int last = round + layers;
+    for (; round <= last && round < MAXROUND; round++) {
+      Queue out{(round & 1) ? ctx->d_qB : ctx->d_qA, cnt + 3 + round, qcap};
+      TIMED(GM_T_TRACK, st, launch_track(ctx->P, in, in_count, in_cap, cnt + 1, out, esc, tally, stats, trace, ctx->n_sm, st));
+      TIMED(GM_T_COMPTON, st, launch_compton(ctx->P, out, stats, trace, ctx->n_sm, st));
+      TIMED(GM_T_ESCAPE, st, launch_escape(ctx->P, esc, out, tally, stats, trace, ctx->n_sm, st));
+      in = out.buf; in_count = out.count; in_cap = qcap;
+    }
+    CK(cudaMemcpyAsync(h_counts, cnt, NCNT * sizeof(int), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    for (int r = 0; r < round; r++) if (h_counts[3 + r] > mq) mq = h_counts[3 + r];
+    if (h_counts[2] > ctx->esc_records) mq = qcap + 1;               // cannot happen (esc >= any tracker input)
+    if (mq > qcap || h_counts[3 + round - 1] == 0) break;            // overflow (caller redoes) or drained
+    if (round >= MAXROUND)
+      return fail(ctx, GM_ERR_STATE, "superphotons still re-entering the grid after %d tracker rounds", round);
   }
-  int h_counts[64];
-  CK(cudaMemcpyAsync(h_counts, cnt, 64 * sizeof(int), cudaMemcpyDeviceToHost, st));
-  CK(cudaStreamSynchronize(st));
-  int mq = 0;
-  for (int layer = 0; layer <= layers; layer++) if (h_counts[2 + layer] > mq) mq = h_counts[2 + layer];
   *max_queue = mq;
   return GM_OK;
 }
@@ -455,7 +475,7 @@ int gm_get_stats(gm_ctx* ctx, gm_stats* out) {
   CK(cudaDeviceSynchronize());
   CK(cudaMemcpy(&h, ctx->d_stats, sizeof(h), cudaMemcpyDeviceToHost));
   int64_t* ni = &out->n_primary;
-  for (int i = 0; i < 13; i++) ni[i] = (int64_t)h.n[i];
+  for (int i = 0; i < 15; i++) ni[i] = (int64_t)h.n[i];
   double* sd = &out->sum_w_emit;
   for (int i = 0; i < 11; i++) sd[i] = h.s[i];
   return GM_OK;

@@ -78,11 +78,11 @@ static_assert(sizeof(Photon) == 160, "Photon record must be 160 bytes");
 
 // per-run device accumulators
 struct DevStats {
-  unsigned long long n[13];
+  unsigned long long n[15];
   double s[11];
 };
 enum { SN_PRIMARY = 0, SN_SPAWNED, SN_RECORDED, SN_HORIZON, SN_ROUL_KILLED, SN_ROUL_SURV, SN_MAXSTEP,
-       SN_OUTOFRANGE, SN_STEPS, SN_VITERS, SN_VCAPPED, SN_BADSCAT, SN_ANALOG };
+       SN_OUTOFRANGE, SN_STEPS, SN_VITERS, SN_VCAPPED, SN_BADSCAT, SN_ANALOG, SN_STEPS_FREE, SN_REENTER };
 enum { SS_EMIT = 0, SS_REC, SS_HORIZON, SS_ROUL_KILLED, SS_ROUL_GAIN, SS_OUTOFRANGE, SS_MAXSTEP,
        SS_ABSORBED, SS_WE_EMIT, SS_WE_REC, SS_BAD };
 

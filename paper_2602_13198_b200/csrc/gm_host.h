@@ -39,10 +39,14 @@ cudaError_t launch_emit(const DevParams& P, const ZoneArrays& Z, long nz, long l
                         const long long* d_ids /* or nullptr: ids = first + i */, Photon* out, int* out_count,
                         DevStats* stats, gm_emit_rec* emit_out /* or nullptr */, bool with_root,
                         cudaStream_t st);
-// track every photon of `in` (count read from device) to completion; scattering events append
-// proto-children (parent state at the event) to `out`
+// track every photon of `in` (count read from device) until it stops or leaves the grid outwards; scattering
+// events append proto-children (parent state at the event) to `out`, leavers go to `esc` (count reset here)
 cudaError_t launch_track(const DevParams& P, const Photon* in, const int* in_count, int in_capacity,
-                         int* work_counter, Queue out, Tally tally, DevStats* stats, TraceBuf trace, int n_sm, cudaStream_t st);
+                         int* work_counter, Queue out, Queue esc, Tally tally, DevStats* stats, TraceBuf trace,
+                         int n_sm, cudaStream_t st);
+// free flight of the leavers to r_max (record) ; a superphoton that re-enters the grid is appended to `ret`
+cudaError_t launch_escape(const DevParams& P, Queue esc, Queue ret, Tally tally, DevStats* stats, TraceBuf trace,
+                          int n_sm, cudaStream_t st);
 // turn the proto-children of `q` into scattered superphotons in place (one Compton event each)
 cudaError_t launch_compton(const DevParams& P, Queue q, DevStats* stats, TraceBuf trace, int n_sm,
                            cudaStream_t st);

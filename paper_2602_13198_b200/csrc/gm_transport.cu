@@ -140,23 +140,62 @@ __global__ void __launch_bounds__(128) emit_kernel(const DevParams P, ZoneArrays
 
 // =====================================================================================================
 // S6-S10, S12: tracker
+//
+// Two kernels share the step:
+//  track_kernel   superphotons inside the fluid grid (or heading into it / into the hole): full step =
+//                 push + gather + plasma state + opacities + absorption + scattering test.
+//  escape_kernel  superphotons that left the grid outwards (x1 >= x1hi, k^1 > 0): nothing but vacuum
+//                 lies ahead, so the step is the geodesic push alone, at a third of the registers.
+// A warp of the tracker keeps its 32 lanes in lock step: one loop iteration = one geodesic step of every
+// lane; stopped lanes are refilled together from a per-warp shared-memory stage that is loaded 32
+// records (5 KB, contiguous) at a time; rare outcomes (record, kill, roulette) sit in out-of-line
+// functions so that the hot loop stays small enough for the instruction cache.
 // =====================================================================================================
 constexpr int TRACK_THREADS = 128;
+constexpr int TRACK_WARPS = TRACK_THREADS / 32;
+constexpr int PH_U4 = sizeof(Photon) / 16;          // 10 x 16 B per record
 
+struct Lane {                                       // registers of the current superphoton
+  double x[4], k[4], a[4], w, nua_a, nua_s, bias;
+  uint32_t id0, id1, id2, nstep, jscat;
+  int nsc, root, flags;
+};
+
+__device__ __forceinline__ void lane_load(Lane& L, const Photon* p) {
+  const double2* p2 = reinterpret_cast<const double2*>(p);
+  double2 v0 = p2[0], v1 = p2[1], v2 = p2[2], v3 = p2[3], v4 = p2[4], v5 = p2[5], v6 = p2[6], v7 = p2[7];
+  const uint4 m0 = reinterpret_cast<const uint4*>(p)[8], m1 = reinterpret_cast<const uint4*>(p)[9];
+  L.x[0] = v0.x; L.x[1] = v0.y; L.x[2] = v1.x; L.x[3] = v1.y;
+  L.k[0] = v2.x; L.k[1] = v2.y; L.k[2] = v3.x; L.k[3] = v3.y;
+  L.a[0] = v4.x; L.a[1] = v4.y; L.a[2] = v5.x; L.a[3] = v5.y;
+  L.w = v6.x; L.nua_a = v6.y; L.nua_s = v7.x; L.bias = v7.y;
+  L.id0 = m0.x; L.id1 = m0.y; L.id2 = m0.z; L.nstep = m0.w;
+  L.nsc = (int)m1.x; L.jscat = m1.y; L.root = (int)m1.z; L.flags = (int)m1.w;
+}
+__device__ __forceinline__ void lane_store(const Lane& L, Photon* c) {
+  double2* c2 = reinterpret_cast<double2*>(c);
+  c2[0] = make_double2(L.x[0], L.x[1]); c2[1] = make_double2(L.x[2], L.x[3]);
+  c2[2] = make_double2(L.k[0], L.k[1]); c2[3] = make_double2(L.k[2], L.k[3]);
+  c2[4] = make_double2(L.a[0], L.a[1]); c2[5] = make_double2(L.a[2], L.a[3]);
+  c2[6] = make_double2(L.w, L.nua_a); c2[7] = make_double2(L.nua_s, L.bias);
+  reinterpret_cast<uint4*>(c)[8] = make_uint4(L.id0, L.id1, L.id2, L.nstep);
+  reinterpret_cast<uint4*>(c)[9] = make_uint4((uint32_t)L.nsc, L.jscat, (uint32_t)L.root, (uint32_t)L.flags);
+}
+
+// ---- rare outcomes, out of line ---------------------------------------------------------------------
 template <bool KERR>
-__device__ __forceinline__ void record_photon(const DevParams& P, const double x[4], const double k[4], double w,
-                                              int root, int flags, unsigned nstep, int nsc, unsigned jscat,
-                                              const Tally& tally, DevStats* stats, const TraceBuf& trace) {
+__device__ __noinline__ void record_photon(const DevParams& P, const Lane& L, const Tally& tally, DevStats* stats,
+                                           const TraceBuf& trace) {
   Geom G;
-  geom_at<KERR, false>(P, x[1], x[2], G, nullptr);
-  const double E = -(G.g00 * k[0] + G.g01 * k[1] + G.g03 * k[3]);     // -k_t, conserved (O9)
+  geom_at<KERR, false>(P, L.x[1], L.x[2], G, nullptr);
+  const double E = -(G.g00 * L.k[0] + G.g01 * L.k[1] + G.g03 * L.k[3]);     // -k_t, conserved (O9)
   int ith = -1, inu = -1;
   bool ok = false;
   if (E > 0.0 && isfinite(E)) {
     double fj = floor(log(E * C_MEC2_H / P.nu_lo) * P.inv_db);
     if (fj >= 0.0 && fj < (double)P.n_nu) {
-      double s2p = sinpi(2.0 * x[2]);
-      double th = C_PI * x[2] + 0.5 * (1.0 - P.hslope) * s2p;
+      double s2p = sinpi(2.0 * L.x[2]);
+      double th = C_PI * L.x[2] + 0.5 * (1.0 - P.hslope) * s2p;
       th = fmod(th, 2.0 * C_PI);
       if (th < 0.0) th += 2.0 * C_PI;
       if (th > C_PI) th = 2.0 * C_PI - th;
@@ -172,33 +211,60 @@ __device__ __forceinline__ void record_photon(const DevParams& P, const double x
     }
   }
   if (ok) {
-    const double wE = w * E;
-    tally_add(tally, ith * P.n_nu + inu, wE, w);
+    const double wE = L.w * E;
+    tally_add(tally, ith * P.n_nu + inu, wE, L.w);
     atomicAdd(&stats->n[SN_RECORDED], 1ull);
-    atomicAdd(&stats->s[SS_REC], w);
+    atomicAdd(&stats->s[SS_REC], L.w);
     atomicAdd(&stats->s[SS_WE_REC], wE);
-    if (trace.rec && root >= 0) atomicAdd(&trace.rec[root].fam_wE, wE);
+    if (trace.rec && L.root >= 0) atomicAdd(&trace.rec[L.root].fam_wE, wE);
   } else {
     atomicAdd(&stats->n[SN_OUTOFRANGE], 1ull);
-    atomicAdd(&stats->s[SS_OUTOFRANGE], w);
+    atomicAdd(&stats->s[SS_OUTOFRANGE], L.w);
   }
-  if (trace.rec && root >= 0 && (flags & FLAG_ROOT)) {
-    gm_trace_rec* r = &trace.rec[root];
-    for (int m = 0; m < 4; m++) { r->x[m] = x[m]; r->k[m] = k[m]; }
-    r->w = w; r->E_inf = E; r->nstep = nstep; r->fate = ok ? GM_FATE_RECORDED : GM_FATE_OUTOFRANGE;
-    r->nsc = nsc; r->ith = ith; r->inu = inu; r->jscat = jscat; r->pad_ = 0;
+  if (trace.rec && L.root >= 0 && (L.flags & FLAG_ROOT)) {
+    gm_trace_rec* r = &trace.rec[L.root];
+    for (int m = 0; m < 4; m++) { r->x[m] = L.x[m]; r->k[m] = L.k[m]; }
+    r->w = L.w; r->E_inf = E; r->nstep = L.nstep; r->fate = ok ? GM_FATE_RECORDED : GM_FATE_OUTOFRANGE;
+    r->nsc = L.nsc; r->ith = ith; r->inu = inu; r->jscat = L.jscat; r->pad_ = 0;
   }
 }
 
-__device__ __forceinline__ void trace_death(const TraceBuf& trace, int root, int flags, const double x[4],
-                                            const double k[4], double w, unsigned nstep, int nsc, unsigned jscat,
-                                            int fate) {
-  if (trace.rec && root >= 0 && (flags & FLAG_ROOT)) {
-    gm_trace_rec* r = &trace.rec[root];
-    for (int m = 0; m < 4; m++) { r->x[m] = x[m]; r->k[m] = k[m]; }
-    r->w = w; r->E_inf = 0.0; r->nstep = nstep; r->fate = fate; r->nsc = nsc; r->ith = -1; r->inu = -1;
-    r->jscat = jscat; r->pad_ = 0;
+// a superphoton that stops without being recorded: counters + optional trace
+__device__ __noinline__ void kill_photon(const Lane& L, int fate, int n_idx, int s_idx, DevStats* stats,
+                                         const TraceBuf& trace) {
+  atomicAdd(&stats->n[n_idx], 1ull);
+  if (s_idx >= 0) atomicAdd(&stats->s[s_idx], L.w);
+  if (trace.rec && L.root >= 0 && (L.flags & FLAG_ROOT)) {
+    gm_trace_rec* r = &trace.rec[L.root];
+    for (int m = 0; m < 4; m++) { r->x[m] = L.x[m]; r->k[m] = L.k[m]; }
+    r->w = L.w; r->E_inf = 0.0; r->nstep = L.nstep; r->fate = fate; r->nsc = L.nsc; r->ith = -1; r->inu = -1;
+    r->jscat = L.jscat; r->pad_ = 0;
   }
+}
+
+// weight roulette (G15); returns false when the superphoton is killed
+__device__ __noinline__ bool roulette(const DevParams& P, Lane& L, double ur, DevStats* stats, const TraceBuf& trace) {
+  if (ur < P.inv_roulette) {
+    atomicAdd(&stats->n[SN_ROUL_SURV], 1ull);
+    atomicAdd(&stats->s[SS_ROUL_GAIN], L.w * (P.roulette - 1.0));
+    L.w *= P.roulette;
+    return true;
+  }
+  kill_photon(L, GM_FATE_ROULETTE, SN_ROUL_KILLED, SS_ROUL_KILLED, stats, trace);
+  return false;
+}
+
+// start-of-step tests shared by both kernels (G14, polar reflection of G4).  Returns true when the
+// superphoton stopped (recorded or killed).
+template <bool KERR>
+__device__ __forceinline__ bool stop_tests(const DevParams& P, Lane& L, const Tally& tally, DevStats* stats,
+                                           const TraceBuf& trace) {
+  if (L.x[2] < 0.0) { L.x[2] = -L.x[2]; L.k[2] = -L.k[2]; L.a[2] = -L.a[2]; L.x[3] += C_PI; }
+  if (L.x[2] > 1.0) { L.x[2] = 2.0 - L.x[2]; L.k[2] = -L.k[2]; L.a[2] = -L.a[2]; L.x[3] += C_PI; }
+  if (L.x[1] >= P.lnr_max) { record_photon<KERR>(P, L, tally, stats, trace); return true; }
+  if (KERR && L.x[1] <= P.lnr_hor) { kill_photon(L, GM_FATE_HORIZON, SN_HORIZON, SS_HORIZON, stats, trace); return true; }
+  if ((long long)L.nstep >= P.max_steps) { kill_photon(L, GM_FATE_MAXSTEP, SN_MAXSTEP, SS_MAXSTEP, stats, trace); return true; }
+  return false;
 }
 
 #ifndef GM_TRACK_MINBLOCKS
@@ -208,140 +274,142 @@ __device__ __forceinline__ void trace_death(const TraceBuf& trace, int root, int
 template <bool KERR, bool THREED>
 __global__ void __launch_bounds__(TRACK_THREADS, GM_TRACK_MINBLOCKS)
 track_kernel(const DevParams P, const Photon* __restrict__ in, const int* __restrict__ in_count, int in_capacity,
-             int* work_counter, Queue out, Tally tally, DevStats* stats, TraceBuf trace) {
+             int* work_counter, Queue out, Queue esc, Tally tally, DevStats* stats, TraceBuf trace) {
+  __shared__ uint4 s_stage[TRACK_WARPS][32 * PH_U4];      // 4 x 5 KB: next 32 records of each warp
   const int n_in = min(*in_count, in_capacity);
-  // registers of the current superphoton
-  double x[4], k[4], a[4], w = 0.0, nua_a = 0.0, nua_s = 0.0, bias = 1.0;
-  uint32_t id0 = 0, id1 = 0, id2 = 0, nstep = 0, jscat = 0;
-  int nsc = 0, root = -1, flags = 0;
-  bool have = false;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  const unsigned lt_mask = (1u << lane) - 1u;
+  uint4* stage = s_stage[wid];
+  Lane L;
+  L.w = 0.0; L.nua_a = 0.0; L.nua_s = 0.0; L.bias = 1.0;
+  L.id0 = L.id1 = L.id2 = L.nstep = L.jscat = 0u; L.nsc = 0; L.root = -1; L.flags = 0;
+#pragma unroll
+  for (int m = 0; m < 4; m++) { L.x[m] = 0.0; L.k[m] = 0.0; L.a[m] = 0.0; }
+  bool have = false, want_scat = false;
   int mode = 0;                         // 0 normal step, 1 partial push to a scattering event, 2 redo full step
   double dl = 0.0, ux = 0.0, ev_f = 0.0, ev_b = 1.0, ev_tau = 0.0;
-  bool want_scat = false;
-  // thread-local counters
+  int st_next = 0, st_avail = 0;        // staged records [st_next, st_avail); warp-uniform
+  bool exhausted = false;               // warp-uniform
   unsigned long long c_steps = 0, c_viters = 0;
   double c_absorbed = 0.0;
 
   for (;;) {
-    if (!have) {
-      const int idx = atomicAdd(work_counter, 1);
-      if (idx >= n_in) break;
-      const Photon* p = in + idx;
-      const double2* p2 = reinterpret_cast<const double2*>(p);
-      double2 v0 = p2[0], v1 = p2[1], v2 = p2[2], v3 = p2[3], v4 = p2[4], v5 = p2[5], v6 = p2[6], v7 = p2[7];
-      const uint4 m0 = reinterpret_cast<const uint4*>(p)[8], m1 = reinterpret_cast<const uint4*>(p)[9];
-      x[0] = v0.x; x[1] = v0.y; x[2] = v1.x; x[3] = v1.y;
-      k[0] = v2.x; k[1] = v2.y; k[2] = v3.x; k[3] = v3.y;
-      a[0] = v4.x; a[1] = v4.y; a[2] = v5.x; a[3] = v5.y;
-      w = v6.x; nua_a = v6.y; nua_s = v7.x; bias = v7.y;
-      id0 = m0.x; id1 = m0.y; id2 = m0.z; nstep = m0.w;
-      nsc = (int)m1.x; jscat = m1.y; root = (int)m1.z; flags = (int)m1.w;
-      if (flags & FLAG_DEAD) continue;
-      have = true; mode = 0;
-      want_scat = P.scattering_on != 0 && nsc < P.nsc_max;
+    __syncwarp();
+    // ---- refill the stopped lanes of this warp together ----
+    const unsigned need = __ballot_sync(0xffffffffu, !have);
+    if (need) {
+      if (st_next == st_avail && !exhausted) {
+        int base = 0;
+        if (lane == 0) base = atomicAdd(work_counter, 32);
+        base = __shfl_sync(0xffffffffu, base, 0);
+        const int cnt = min(32, n_in - base);
+        if (cnt <= 0) {
+          exhausted = true;
+        } else {
+          const uint4* src = reinterpret_cast<const uint4*>(in + base);
+          for (int i = lane; i < cnt * PH_U4; i += 32) stage[i] = __ldg(src + i);
+          st_next = 0; st_avail = cnt;
+        }
+        __syncwarp();
+      }
+      const int left = st_avail - st_next;
+      if (left > 0) {
+        const int rank = __popc(need & lt_mask);
+        if (!have && rank < left) {
+          lane_load(L, reinterpret_cast<const Photon*>(stage) + st_next + rank);
+          if (!(L.flags & FLAG_DEAD)) {
+            have = true; mode = 0;
+            want_scat = P.scattering_on != 0 && L.nsc < P.nsc_max;
+          }
+        }
+        st_next += min(__popc(need), left);
+        __syncwarp();
+      } else if (exhausted && need == 0xffffffffu) {
+        break;
+      }
     }
+    if (!have) continue;
+
     if (mode == 0) {
-      // polar-axis reflection, stop tests (G14), roulette (G15), step size (G16)
-      if (x[2] < 0.0) { x[2] = -x[2]; k[2] = -k[2]; a[2] = -a[2]; x[3] += C_PI; }
-      if (x[2] > 1.0) { x[2] = 2.0 - x[2]; k[2] = -k[2]; a[2] = -a[2]; x[3] += C_PI; }
-      if (x[1] >= P.lnr_max) {
-        record_photon<KERR>(P, x, k, w, root, flags, nstep, nsc, jscat, tally, stats, trace);
-        have = false; continue;
-      }
-      if (KERR && x[1] <= P.lnr_hor) {
-        atomicAdd(&stats->n[SN_HORIZON], 1ull); atomicAdd(&stats->s[SS_HORIZON], w);
-        trace_death(trace, root, flags, x, k, w, nstep, nsc, jscat, GM_FATE_HORIZON);
-        have = false; continue;
-      }
-      if ((long long)nstep >= P.max_steps) {
-        atomicAdd(&stats->n[SN_MAXSTEP], 1ull); atomicAdd(&stats->s[SS_MAXSTEP], w);
-        trace_death(trace, root, flags, x, k, w, nstep, nsc, jscat, GM_FATE_MAXSTEP);
+      if (stop_tests<KERR>(P, L, tally, stats, trace)) { have = false; continue; }
+      if (L.x[1] >= P.x1hi && L.k[1] > 0.0) {              // leaves the grid outwards: free flight
+        const int slot = atomicAdd(esc.count, 1);
+        if (slot < esc.capacity) lane_store(L, esc.buf + slot);
         have = false; continue;
       }
       double ur;
-      uniform_pair(P, TAG_STEP, id0, id1, id2, nstep, ux, ur);
-      if (w < P.w_min) {
-        if (ur < P.inv_roulette) {
-          atomicAdd(&stats->n[SN_ROUL_SURV], 1ull); atomicAdd(&stats->s[SS_ROUL_GAIN], w * (P.roulette - 1.0));
-          w *= P.roulette;
-        } else {
-          atomicAdd(&stats->n[SN_ROUL_KILLED], 1ull); atomicAdd(&stats->s[SS_ROUL_KILLED], w);
-          trace_death(trace, root, flags, x, k, w, nstep, nsc, jscat, GM_FATE_ROULETTE);
-          have = false; continue;
-        }
-      }
-      dl = step_size(P, x, k);
+      uniform_pair(P, TAG_STEP, L.id0, L.id1, L.id2, L.nstep, ux, ur);
+      if (L.w < P.w_min && !roulette(P, L, ur, stats, trace)) { have = false; continue; }
+      dl = step_size(P, L.x, L.k);
     }
     const double dl_eff = (mode == 1) ? ev_f * dl : dl;
     double x1[4], k1[4], a1[4];
     Geom G;
     bool capped;
-    const int it = push<KERR>(P, x, k, a, dl_eff, x1, k1, a1, G, capped);
+    const int it = push<KERR>(P, L.x, L.k, L.a, dl_eff, x1, k1, a1, G, capped);
     Plasma S;
     const bool inplasma = plasma_at<THREED>(P, x1, G, S);
+    double na1 = 0.0, ns1 = 0.0, b1 = 1.0;
+    if (inplasma) opacities(P, k1, G, S, L.nsc, want_scat, na1, ns1, b1);
 
     if (mode == 1) {
       // ---- scattering event at x1 ----
-      if (inplasma && S.ne > 0.0) {
-        c_viters += it; if (capped) atomicAdd(&stats->n[SN_VCAPPED], 1ull);
-        const double w0 = w;
-        w = w0 * exp(-ev_f * ev_tau);                      // Eq. 19 up to the event
-        c_absorbed += w0 - w;
+      if (!(inplasma && S.ne > 0.0)) { mode = 2; continue; }   // event point in vacuum: full step instead (G30)
+      c_viters += it; if (capped) atomicAdd(&stats->n[SN_VCAPPED], 1ull);
+      const double w0 = L.w;
+      const double wev = w0 * exp(-ev_f * ev_tau);           // Eq. 19 up to the event
+      c_absorbed += w0 - wev;
 #pragma unroll
-        for (int m = 0; m < 4; m++) { x[m] = x1[m]; k[m] = k1[m]; a[m] = a1[m]; }
-        const double wc = w / ev_b;                        // child weight w/b
-        const int slot = atomicAdd(out.count, 1);
-        if (slot < out.capacity) {
-          Photon* c = out.buf + slot;
-          double2* c2 = reinterpret_cast<double2*>(c);
-          c2[0] = make_double2(x[0], x[1]); c2[1] = make_double2(x[2], x[3]);
-          c2[2] = make_double2(k[0], k[1]); c2[3] = make_double2(k[2], k[3]);
-          c2[4] = make_double2(0.0, 0.0); c2[5] = make_double2(0.0, 0.0);
-          c2[6] = make_double2(wc, 0.0); c2[7] = make_double2(0.0, 1.0);
-          reinterpret_cast<uint4*>(c)[8] = make_uint4(id0, id1, id2, 0u);
-          reinterpret_cast<uint4*>(c)[9] = make_uint4((uint32_t)nsc, jscat, (uint32_t)root, 0u);
-        }
-        w -= wc;                                           // parent keeps w (1 - 1/b)
-        jscat++;
-        opacities(P, k, G, S, nsc, want_scat, nua_a, nua_s, bias);
-        nstep++; c_steps++;
-        mode = 0;
-        if (!(w > 0.0)) {                                  // analog limit b = 1
-          atomicAdd(&stats->n[SN_ANALOG], 1ull);
-          trace_death(trace, root, flags, x, k, w, nstep, nsc, jscat, GM_FATE_ANALOG);
-          have = false;
-        }
-      } else {
-        mode = 2;                                          // event point in vacuum: take the full step instead
+      for (int m = 0; m < 4; m++) { L.x[m] = x1[m]; L.k[m] = k1[m]; L.a[m] = a1[m]; }
+      const double wc = wev / ev_b;                          // child weight w/b
+      const int slot = atomicAdd(out.count, 1);
+      if (slot < out.capacity) {
+        Photon* c = out.buf + slot;
+        double2* c2 = reinterpret_cast<double2*>(c);
+        c2[0] = make_double2(L.x[0], L.x[1]); c2[1] = make_double2(L.x[2], L.x[3]);
+        c2[2] = make_double2(L.k[0], L.k[1]); c2[3] = make_double2(L.k[2], L.k[3]);
+        c2[4] = make_double2(0.0, 0.0); c2[5] = make_double2(0.0, 0.0);
+        c2[6] = make_double2(wc, 0.0); c2[7] = make_double2(0.0, 1.0);
+        reinterpret_cast<uint4*>(c)[8] = make_uint4(L.id0, L.id1, L.id2, 0u);
+        reinterpret_cast<uint4*>(c)[9] = make_uint4((uint32_t)L.nsc, L.jscat, (uint32_t)L.root, 0u);
+      }
+      L.w = wev - wc;                                        // parent keeps w (1 - 1/b)
+      L.jscat++;
+      L.nua_a = na1; L.nua_s = ns1; L.bias = b1;
+      L.nstep++; c_steps++;
+      mode = 0;
+      if (!(L.w > 0.0)) {                                    // analog limit b = 1
+        kill_photon(L, GM_FATE_ANALOG, SN_ANALOG, -1, stats, trace);
+        have = false;
       }
       continue;
     }
 
-    double na1 = 0.0, ns1 = 0.0, b1 = 1.0;
-    if (inplasma) opacities(P, k1, G, S, nsc, want_scat, na1, ns1, b1);
-    const double tau_a = 0.5 * (nua_a + na1) * P.Cfac * dl;          // Eq. 20
+    const double tau_a = 0.5 * (L.nua_a + na1) * P.Cfac * dl;          // Eq. 20
     if (mode == 0) {
       c_viters += it; if (capped) atomicAdd(&stats->n[SN_VCAPPED], 1ull);
       if (want_scat) {
-        const double tau_s = 0.5 * (nua_s + ns1) * P.Cfac * dl;      // Eq. 25
-        if (tau_s > 0.0) {
-          const double b = 0.5 * (bias + b1);                        // G19
-          const double xr = -log(1.0 - ux);                          // PAPER.md:176
-          if (b * tau_s > xr && w / b >= P.w_min) {
-            mode = 1; ev_f = xr / (b * tau_s); ev_b = b; ev_tau = tau_a;
+        const double tau_s = 0.5 * (L.nua_s + ns1) * P.Cfac * dl;      // Eq. 25
+        const double bt = 0.5 * (L.bias + b1) * tau_s;                 // G19
+        // x_r = -ln(1-u) >= u: the logarithm is needed only when b tau_s exceeds u
+        if (bt > ux) {
+          const double b = 0.5 * (L.bias + b1);
+          const double xr = -log(1.0 - ux);
+          if (bt > xr && L.w / b >= P.w_min) {
+            mode = 1; ev_f = xr / bt; ev_b = b; ev_tau = tau_a;
             continue;
           }
         }
       }
     }
     // ---- commit the step (Eq. 19) ----
-    const double w0 = w;
-    w = w0 * exp(-tau_a);
-    c_absorbed += w0 - w;
+    const double w0 = L.w;
+    L.w = w0 * exp(-tau_a);
+    c_absorbed += w0 - L.w;
 #pragma unroll
-    for (int m = 0; m < 4; m++) { x[m] = x1[m]; k[m] = k1[m]; a[m] = a1[m]; }
-    nua_a = na1; nua_s = ns1; bias = b1;
-    nstep++; c_steps++;
+    for (int m = 0; m < 4; m++) { L.x[m] = x1[m]; L.k[m] = k1[m]; L.a[m] = a1[m]; }
+    L.nua_a = na1; L.nua_s = ns1; L.bias = b1;
+    L.nstep++; c_steps++;
     mode = 0;
   }
   // flush thread-local counters
@@ -350,10 +418,62 @@ track_kernel(const DevParams P, const Photon* __restrict__ in, const int* __rest
     c_viters += __shfl_xor_sync(0xffffffffu, c_viters, o);
   }
   c_absorbed = warp_sum(c_absorbed);
-  if ((threadIdx.x & 31) == 0) {
+  if (lane == 0) {
     stat_add_n(stats, SN_STEPS, c_steps);
     stat_add_n(stats, SN_VITERS, c_viters);
     stat_add_s(stats, SS_ABSORBED, c_absorbed);
+  }
+}
+
+// ---- free flight beyond the grid: the same step with vacuum ahead (tau_a = tau_s = 0) -----------------
+// A superphoton that comes back below x1hi (possible only for grids that end inside the photon orbit) is
+// appended to `ret` as a complete record and tracked by the next tracker launch.
+template <bool KERR>
+#ifndef GM_ESC_MINBLOCKS
+#define GM_ESC_MINBLOCKS 4
+#endif
+__global__ void __launch_bounds__(128, GM_ESC_MINBLOCKS)
+escape_kernel(const DevParams P, Queue esc, Queue ret, Tally tally, DevStats* stats, TraceBuf trace) {
+  const int n = min(*esc.count, esc.capacity);
+  unsigned long long c_steps = 0, c_viters = 0, c_capped = 0;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+    Lane L;
+    lane_load(L, esc.buf + i);
+    for (;;) {
+      if (stop_tests<KERR>(P, L, tally, stats, trace)) break;
+      if (L.x[1] < P.x1hi) {                                 // back inside the grid
+        L.nua_a = 0.0; L.nua_s = 0.0; L.bias = 1.0;          // opacities at a vacuum point
+        const int slot = atomicAdd(ret.count, 1);
+        if (slot < ret.capacity) lane_store(L, ret.buf + slot);
+        atomicAdd(&stats->n[SN_REENTER], 1ull);
+        break;
+      }
+      if (L.w < P.w_min) {
+        double ux, ur;
+        uniform_pair(P, TAG_STEP, L.id0, L.id1, L.id2, L.nstep, ux, ur);
+        if (!roulette(P, L, ur, stats, trace)) break;
+      }
+      const double dl = step_size(P, L.x, L.k);
+      double x1[4], k1[4], a1[4];
+      Geom G;
+      bool capped;
+      c_viters += push<KERR>(P, L.x, L.k, L.a, dl, x1, k1, a1, G, capped);
+      c_capped += capped ? 1 : 0;
+#pragma unroll
+      for (int m = 0; m < 4; m++) { L.x[m] = x1[m]; L.k[m] = k1[m]; L.a[m] = a1[m]; }
+      L.nstep++; c_steps++;
+    }
+  }
+  for (int o = 16; o > 0; o >>= 1) {
+    c_steps += __shfl_xor_sync(0xffffffffu, c_steps, o);
+    c_viters += __shfl_xor_sync(0xffffffffu, c_viters, o);
+    c_capped += __shfl_xor_sync(0xffffffffu, c_capped, o);
+  }
+  if ((threadIdx.x & 31) == 0) {
+    stat_add_n(stats, SN_STEPS, c_steps);
+    stat_add_n(stats, SN_STEPS_FREE, c_steps);
+    stat_add_n(stats, SN_VITERS, c_viters);
+    stat_add_n(stats, SN_VCAPPED, c_capped);
   }
 }
 
@@ -632,12 +752,22 @@ cudaError_t launch_emit(const DevParams& P, const ZoneArrays& Z, long nz, long l
 }
 
 cudaError_t launch_track(const DevParams& P, const Photon* in, const int* in_count, int in_capacity,
-                         int* work_counter, Queue out, Tally tally, DevStats* stats, TraceBuf trace, int n_sm,
-                         cudaStream_t st) {
+                         int* work_counter, Queue out, Queue esc, Tally tally, DevStats* stats, TraceBuf trace,
+                         int n_sm, cudaStream_t st) {
   cudaError_t e = cudaMemsetAsync(work_counter, 0, sizeof(int), st);
   if (e != cudaSuccess) return e;
+  if ((e = cudaMemsetAsync(esc.count, 0, sizeof(int), st)) != cudaSuccess) return e;
   const int grid = n_sm * GM_TRACK_MINBLOCKS;
-  GM_DISPATCH(track_kernel, grid, TRACK_THREADS, st, P, in, in_count, in_capacity, work_counter, out, tally, stats, trace);
+  GM_DISPATCH(track_kernel, grid, TRACK_THREADS, st, P, in, in_count, in_capacity, work_counter, out, esc, tally, stats,
+              trace);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_escape(const DevParams& P, Queue esc, Queue ret, Tally tally, DevStats* stats, TraceBuf trace,
+                          int n_sm, cudaStream_t st) {
+  const int grid = n_sm * GM_ESC_MINBLOCKS;
+  if (P.metric_kind == 1) escape_kernel<true><<<grid, 128, 0, st>>>(P, esc, ret, tally, stats, trace);
+  else escape_kernel<false><<<grid, 128, 0, st>>>(P, esc, ret, tally, stats, trace);
   return cudaGetLastError();
 }
 
