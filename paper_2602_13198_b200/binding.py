@@ -12,7 +12,8 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libgpumonty_b200.so")
+# GPUMONTY_B200_LIB selects another build of the same library (tuning experiments: launch bounds etc.)
+LIB_PATH = os.environ.get("GPUMONTY_B200_LIB") or os.path.join(_HERE, "libgpumonty_b200.so")
 
 GM_ABI_VERSION = 1
 TABLE_LNK2, TABLE_LNF, TABLE_LNSIGH, TABLE_LNW, TABLE_NEXP, TABLE_QMAX = range(6)

@@ -129,6 +129,7 @@ static void fill_dev_params(gm_ctx* c) {
   P.hslope = p.hslope;
   P.startx1 = p.startx[1]; P.startx2 = p.startx[2]; P.startx3 = p.startx[3];
   P.dx1 = p.dx[1]; P.dx2 = p.dx[2]; P.dx3 = p.dx[3];
+  P.inv_dx1 = 1.0 / p.dx[1]; P.inv_dx2 = 1.0 / p.dx[2]; P.inv_dx3 = 1.0 / p.dx[3];
   P.x1lo = p.startx[1]; P.x1hi = p.startx[1] + p.n1 * p.dx[1];
   P.n1 = p.n1; P.n2 = p.n2; P.n3 = p.n3; P.metric_kind = p.metric_kind;
   P.L_unit = p.L_unit;

@@ -37,7 +37,7 @@ constexpr uint32_t TAG_ZONE = 0x5a4f4e45u, TAG_EMIT = 0x454d4954u, TAG_STEP = 0x
 struct DevParams {
   // geometry / grid
   double a_spin, hslope;
-  double startx1, startx2, startx3, dx1, dx2, dx3;
+  double startx1, startx2, startx3, dx1, dx2, dx3, inv_dx1, inv_dx2, inv_dx3;
   double x1lo, x1hi;
   int n1, n2, n3, metric_kind;
   // units

@@ -242,16 +242,18 @@ __device__ __noinline__ void kill_photon(const Lane& L, int fate, int n_idx, int
   }
 }
 
-// weight roulette (G15); returns false when the superphoton is killed
-__device__ __noinline__ bool roulette(const DevParams& P, Lane& L, double ur, DevStats* stats, const TraceBuf& trace) {
+// weight roulette (G15); returns the new weight, or a negative number when the superphoton is killed.
+// The out-of-line functions get a COPY of the lane state (their argument has its address taken; the
+// live state must stay in registers).
+__device__ __noinline__ double roulette(const DevParams& P, const Lane& L, double ur, DevStats* stats,
+                                        const TraceBuf& trace) {
   if (ur < P.inv_roulette) {
     atomicAdd(&stats->n[SN_ROUL_SURV], 1ull);
     atomicAdd(&stats->s[SS_ROUL_GAIN], L.w * (P.roulette - 1.0));
-    L.w *= P.roulette;
-    return true;
+    return L.w * P.roulette;
   }
   kill_photon(L, GM_FATE_ROULETTE, SN_ROUL_KILLED, SS_ROUL_KILLED, stats, trace);
-  return false;
+  return -1.0;
 }
 
 // start-of-step tests shared by both kernels (G14, polar reflection of G4).  Returns true when the
@@ -261,9 +263,13 @@ __device__ __forceinline__ bool stop_tests(const DevParams& P, Lane& L, const Ta
                                            const TraceBuf& trace) {
   if (L.x[2] < 0.0) { L.x[2] = -L.x[2]; L.k[2] = -L.k[2]; L.a[2] = -L.a[2]; L.x[3] += C_PI; }
   if (L.x[2] > 1.0) { L.x[2] = 2.0 - L.x[2]; L.k[2] = -L.k[2]; L.a[2] = -L.a[2]; L.x[3] += C_PI; }
-  if (L.x[1] >= P.lnr_max) { record_photon<KERR>(P, L, tally, stats, trace); return true; }
-  if (KERR && L.x[1] <= P.lnr_hor) { kill_photon(L, GM_FATE_HORIZON, SN_HORIZON, SS_HORIZON, stats, trace); return true; }
-  if ((long long)L.nstep >= P.max_steps) { kill_photon(L, GM_FATE_MAXSTEP, SN_MAXSTEP, SS_MAXSTEP, stats, trace); return true; }
+  if (L.x[1] >= P.lnr_max) { const Lane T = L; record_photon<KERR>(P, T, tally, stats, trace); return true; }
+  if (KERR && L.x[1] <= P.lnr_hor) {
+    const Lane T = L; kill_photon(T, GM_FATE_HORIZON, SN_HORIZON, SS_HORIZON, stats, trace); return true;
+  }
+  if ((long long)L.nstep >= P.max_steps) {
+    const Lane T = L; kill_photon(T, GM_FATE_MAXSTEP, SN_MAXSTEP, SS_MAXSTEP, stats, trace); return true;
+  }
   return false;
 }
 
@@ -273,7 +279,7 @@ __device__ __forceinline__ bool stop_tests(const DevParams& P, Lane& L, const Ta
 
 template <bool KERR, bool THREED>
 __global__ void __launch_bounds__(TRACK_THREADS, GM_TRACK_MINBLOCKS)
-track_kernel(const DevParams P, const Photon* __restrict__ in, const int* __restrict__ in_count, int in_capacity,
+track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in, const int* __restrict__ in_count, int in_capacity,
              int* work_counter, Queue out, Queue esc, Tally tally, DevStats* stats, TraceBuf trace) {
   __shared__ uint4 s_stage[TRACK_WARPS][32 * PH_U4];      // 4 x 5 KB: next 32 records of each warp
   const int n_in = min(*in_count, in_capacity);
@@ -339,18 +345,29 @@ track_kernel(const DevParams P, const Photon* __restrict__ in, const int* __rest
       }
       double ur;
       uniform_pair(P, TAG_STEP, L.id0, L.id1, L.id2, L.nstep, ux, ur);
-      if (L.w < P.w_min && !roulette(P, L, ur, stats, trace)) { have = false; continue; }
+      if (L.w < P.w_min) {
+        const Lane T = L;
+        L.w = roulette(P, T, ur, stats, trace);
+        if (L.w < 0.0) { have = false; continue; }
+      }
       dl = step_size(P, L.x, L.k);
     }
     const double dl_eff = (mode == 1) ? ev_f * dl : dl;
     double x1[4], k1[4], a1[4];
     Geom G;
     bool capped;
-    const int it = push<KERR>(P, L.x, L.k, L.a, dl_eff, x1, k1, a1, G, capped);
+    push_position(L.x, L.k, L.a, dl_eff, x1);
+    // the gather needs only the position: issue it before the metric work of the push so that the loads fly
+    // while the FP64 pipe is busy (S8)
+    double pr[8];
+    const bool inplasma = interp_prim<THREED>(P, x1, pr) && pr[0] > 0.0;
+    const int it = push_wavevector<KERR>(P, L.k, L.a, dl_eff, x1, k1, a1, G, capped);
     Plasma S;
-    const bool inplasma = plasma_at<THREED>(P, x1, G, S);
     double na1 = 0.0, ns1 = 0.0, b1 = 1.0;
-    if (inplasma) opacities(P, k1, G, S, L.nsc, want_scat, na1, ns1, b1);
+    if (inplasma) {
+      plasma_from_prim(P, G, pr, S);
+      opacities(P, k1, G, S, L.nsc, want_scat, na1, ns1, b1);
+    }
 
     if (mode == 1) {
       // ---- scattering event at x1 ----
@@ -379,7 +396,8 @@ track_kernel(const DevParams P, const Photon* __restrict__ in, const int* __rest
       L.nstep++; c_steps++;
       mode = 0;
       if (!(L.w > 0.0)) {                                    // analog limit b = 1
-        kill_photon(L, GM_FATE_ANALOG, SN_ANALOG, -1, stats, trace);
+        const Lane T = L;
+        kill_photon(T, GM_FATE_ANALOG, SN_ANALOG, -1, stats, trace);
         have = false;
       }
       continue;
@@ -403,9 +421,11 @@ track_kernel(const DevParams P, const Photon* __restrict__ in, const int* __rest
       }
     }
     // ---- commit the step (Eq. 19) ----
-    const double w0 = L.w;
-    L.w = w0 * exp(-tau_a);
-    c_absorbed += w0 - L.w;
+    if (tau_a != 0.0) {                                    // exp(-0) = 1 exactly: cold and vacuum steps skip it
+      const double w0 = L.w;
+      L.w = w0 * exp(-tau_a);
+      c_absorbed += w0 - L.w;
+    }
 #pragma unroll
     for (int m = 0; m < 4; m++) { L.x[m] = x1[m]; L.k[m] = k1[m]; L.a[m] = a1[m]; }
     L.nua_a = na1; L.nua_s = ns1; L.bias = b1;
@@ -433,7 +453,7 @@ template <bool KERR>
 #define GM_ESC_MINBLOCKS 4
 #endif
 __global__ void __launch_bounds__(128, GM_ESC_MINBLOCKS)
-escape_kernel(const DevParams P, Queue esc, Queue ret, Tally tally, DevStats* stats, TraceBuf trace) {
+escape_kernel(const __grid_constant__ DevParams P, Queue esc, Queue ret, Tally tally, DevStats* stats, TraceBuf trace) {
   const int n = min(*esc.count, esc.capacity);
   unsigned long long c_steps = 0, c_viters = 0, c_capped = 0;
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
@@ -451,7 +471,9 @@ escape_kernel(const DevParams P, Queue esc, Queue ret, Tally tally, DevStats* st
       if (L.w < P.w_min) {
         double ux, ur;
         uniform_pair(P, TAG_STEP, L.id0, L.id1, L.id2, L.nstep, ux, ur);
-        if (!roulette(P, L, ur, stats, trace)) break;
+        const Lane T = L;
+        L.w = roulette(P, T, ur, stats, trace);
+        if (L.w < 0.0) break;
       }
       const double dl = step_size(P, L.x, L.k);
       double x1[4], k1[4], a1[4];
