@@ -35,9 +35,12 @@ from paper_2602_13198_b200.shard import rank_seed, reduce_tally  # noqa: E402
 
 METRIC = "superphotons/s tracked (incl. scattering)"
 UNIT = "superphotons/s"
-# algorithmic FP64 flop per geodesic step of the tracker (dadd + dmul + 2 dfma thread
-# instructions per committed step, counted once with ncu on each workload class and then frozen)
-FLOP_PER_STEP = {"flat": 1.30e3, "kerr": 2.20e3}
+# algorithmic FP64 flop per geodesic step (dadd + dmul + 2 dfma predicated-on thread
+# instructions of the kernel divided by the steps it committed, counted with ncu on each workload class --
+# profiles/r01b_flop_per_step.md -- and then frozen).  "track": in-grid step of track_kernel; "escape":
+# free-flight step of escape_kernel.
+FLOP_PER_STEP = {"flat": {"track": 853.0, "escape": 223.0}, "kerr": {"track": 877.0, "escape": 434.0},
+                 "kerr3d": {"track": 877.0, "escape": 434.0}}
 WORKLOAD_NAMES = {0: "cfg0 thin synchrotron sphere 32x16, Ns=1e5", 1: "cfg1 scattering sphere 32x16, Ns=1e6",
                   2: "cfg2 Kerr FM torus 256x256, Ns=1e7", 3: "cfg3 3-D perturbed torus 192x128x128, Ns=1e7",
                   4: "cfg4 Kerr torus x1e3 density (analog scattering), Ns=1e6"}
@@ -225,10 +228,12 @@ def main():
 
     if rank == 0:
         value = total / (ms_step * 1e-3)
-        kind = "kerr" if p["metric_kind"] == 1 else "flat"
+        kind = ("kerr3d" if p["n3"] > 1 else "kerr") if p["metric_kind"] == 1 else "flat"
         n_track_launches = max(1, tm["track"][1])
         steps_track = st["n_steps_total"] - st["n_steps_free"]      # steps taken inside track_kernel (this rank, last timed step)
-        flops = steps_track * FLOP_PER_STEP[kind]
+        flops = steps_track * FLOP_PER_STEP[kind]["track"]
+        esc_ms = tm["escape"][0] / args.steps
+        esc_tflops = st["n_steps_free"] * FLOP_PER_STEP[kind]["escape"] / max(esc_ms * 1e-3, 1e-9) / 1e12
         track_ms_per_step = tm["track"][0] / args.steps
         peak_meas, _ = gm.fp64_peak()
         achieved = flops / (track_ms_per_step * 1e-3) / 1e12
@@ -249,7 +254,9 @@ def main():
             "roofline": {"bound": "alu", "kernel": "track_kernel", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                          "frac": achieved / peak, "traffic": None,
                          "peak_source": "DFMA-chain microbenchmark run in this process (gm_fp64_peak); nominal 2*64*148*1.965 GHz = 37.2",
-                         "flop_per_step": FLOP_PER_STEP[kind], "track_ms_per_step": track_ms_per_step,
+                         "flop_per_step": FLOP_PER_STEP[kind]["track"], "track_ms_per_step": track_ms_per_step,
+                         "escape_kernel": {"achieved": esc_tflops, "frac": esc_tflops / peak, "ms_per_step": esc_ms,
+                                           "flop_per_step": FLOP_PER_STEP[kind]["escape"]},
                          "track_launches_per_step": n_track_launches // max(1, args.steps),
                          "track_share_of_step": track_ms_per_step / ms_step,
                          "kernel_ms_per_step": {k: v[0] / args.steps for k, v in tm.items()}},

@@ -376,6 +376,43 @@ def test_superphotons_reentering_the_grid_from_free_flight(gm, scattering):
     _compare_traces(o, g, ids, fork_budget=5e-3)
 
 
+def _full_size_checks(gm, p, prim, n_sample, seed):
+    """Full-size run in the launch configuration bench.py times: counts bit-exact, sampled histories against the
+    oracle one by one, and the properties that hold at any size (weight bookkeeping, tally totals)."""
+    o, g = _pair(gm, p, prim)
+    assert np.array_equal(o.zone_counts(), g.zone_counts())
+    g.run()
+    sg = g.stats()
+    A, Q, W, n = g.tally()
+    assert n.sum() == sg["n_recorded"]
+    assert W.sum() == pytest.approx(sg["sum_w_rec"], rel=1e-9) and A.sum() == pytest.approx(sg["sum_wE_rec"], rel=1e-9)
+    assert sg["n_primary"] == g.n_primaries and sg["n_maxstep"] == 0 and sg["n_bad_scatter"] == 0
+    # every superphoton ends exactly once
+    ends = (sg["n_recorded"] + sg["n_horizon"] + sg["n_roulette_killed"] + sg["n_outofrange"] + sg["n_maxstep"] +
+            sg["n_analog_killed"])
+    assert ends == sg["n_primary"] + sg["n_spawned"]
+    # photon number (PAPER.md:148: a scattering only moves weight between parent and child)
+    out = (sg["sum_w_rec"] + sg["sum_w_horizon"] + sg["sum_w_roulette_killed"] - sg["sum_w_roulette_gain"] +
+           sg["sum_w_outofrange"] + sg["sum_w_maxstep"] + sg["sum_w_absorbed"] + sg["sum_w_bad"])
+    assert out == pytest.approx(sg["sum_w_emit"], rel=1e-9)
+    ids = np.sort(np.random.default_rng(seed).choice(g.n_primaries, n_sample, replace=False))
+    _compare_traces(o, g, ids, fork_budget=5e-3)
+    return sg
+
+
+def test_full_size_config2(gm):
+    """BASELINE configs[2] as bench.py runs it: 256x256 Kerr torus, N_s = 1e7 (3.6e6 primaries, 2.5e7 scattered)."""
+    p, prim = wl.config2()
+    sg = _full_size_checks(gm, p, prim, 3000, 21)
+    assert sg["n_spawned"] > 5 * sg["n_primary"]
+
+
+def test_full_size_config1(gm):
+    """BASELINE configs[1] at N_s = 1e6."""
+    p, prim = wl.config1()
+    _full_size_checks(gm, p, prim, 3000, 22)
+
+
 def test_batching_and_queue_overflow_recovery(gm):
     """S13: id-range batches give the same tally as one batch; a queue that is too small makes the driver
     shrink the batch and redo it (nothing dropped), never a silent loss."""
