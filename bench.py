@@ -151,6 +151,8 @@ def main():
     ap.add_argument("--ns", type=float, default=None, help="override N_s of the config")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--phase-pairs", type=int, default=-1, help="hot/cold tracker pass pairs per generation (-1: library default)")
+    ap.add_argument("--k-cold", type=int, default=4, help="cold steps after which a hot pass hands a superphoton over")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -173,6 +175,7 @@ def main():
 
     p, prim = make_workload(args.config, args.ns, rank_seed(1, rank))
     g = gm.GPUMonty(p)
+    g.set_phase_passes(args.phase_pairs, args.k_cold)
     host_grid = torch.from_numpy(prim).pin_memory()
     dev_grid = host_grid.cuda()
     flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.float32, device="cuda")   # > 126 MB L2

@@ -23,7 +23,7 @@ _EVAL_SHAPES = {EVAL_ACCEL: (8, 4), EVAL_GEOM: (4, 33), EVAL_PLASMA: (4, 12), EV
 FATE_ALIVE, FATE_RECORDED, FATE_HORIZON, FATE_ROULETTE, FATE_MAXSTEP, FATE_OUTOFRANGE, FATE_ANALOG = range(7)
 
 EXPORTS = ["gm_create", "gm_destroy", "gm_last_error", "gm_set_grid", "gm_prepare", "gm_get_zone_counts",
-           "gm_get_table", "gm_run", "gm_set_batch", "gm_get_spectrum", "gm_get_tally", "gm_get_stats",
+           "gm_get_table", "gm_run", "gm_set_batch", "gm_set_phase_passes", "gm_get_spectrum", "gm_get_tally", "gm_get_stats",
            "gm_reset_tally", "gm_emit", "gm_trace", "gm_eval", "gm_fp64_peak", "gm_build_tables", "gm_timing", "gm_spectrum_device"]
 
 
@@ -94,6 +94,7 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
     L.gm_get_table.argtypes = [vp, C.c_int, vp, C.c_size_t]
     L.gm_run.argtypes = [vp, C.c_int64, C.c_int64, vp]
     L.gm_set_batch.argtypes = [vp, C.c_int64, C.c_int64]
+    L.gm_set_phase_passes.argtypes = [vp, C.c_int, C.c_int]
     L.gm_get_spectrum.argtypes = [vp, vp, vp, vp]
     L.gm_get_tally.argtypes = [vp, vp, vp, vp, vp]
     L.gm_get_stats.argtypes = [vp, C.POINTER(GmStats)]
@@ -200,6 +201,9 @@ class GPUMonty:
 
     def set_batch(self, batch_primaries=0, queue_records=0):
         self._ck(self.L.gm_set_batch(self.h, int(batch_primaries), int(queue_records)))
+
+    def set_phase_passes(self, pairs=-1, k_cold=4):
+        self._ck(self.L.gm_set_phase_passes(self.h, int(pairs), int(k_cold)))
 
     def run(self, first=0, n=None, stream=None):
         if n is None:

@@ -26,6 +26,8 @@ struct gm_ctx {
   double *d_spec = nullptr;          // [2][nb]
   int* d_counters = nullptr;         // [0] primaries count, [1] queue A count, [2] queue B count, [3] work counter
   Photon *d_prim_ph = nullptr, *d_qA = nullptr, *d_qB = nullptr, *d_esc = nullptr;
+  Photon *d_parkA = nullptr, *d_parkB = nullptr;   // hot/cold pass hand-over queues (esc_records each)
+  int phase_pairs = -1, k_cold = 4;                // -1: automatic (2 for Kerr with a temperature model, else 0)
   long long esc_records = 0;
   long long batch_primaries = 0, queue_records = 0;   // allocated sizes
   long long want_batch = 0, want_queue = 0;
@@ -76,7 +78,8 @@ static int fail(gm_ctx* c, int code, const char* fmt, ...) {
 
 static void free_run_buffers(gm_ctx* c) {
   cudaFree(c->d_prim_ph); cudaFree(c->d_qA); cudaFree(c->d_qB); cudaFree(c->d_esc);
-  c->d_prim_ph = c->d_qA = c->d_qB = c->d_esc = nullptr;
+  cudaFree(c->d_parkA); cudaFree(c->d_parkB);
+  c->d_prim_ph = c->d_qA = c->d_qB = c->d_esc = c->d_parkA = c->d_parkB = nullptr;
   c->batch_primaries = c->queue_records = c->esc_records = 0;
 }
 
@@ -213,7 +216,7 @@ int gm_create(gm_ctx** out, const gm_params* p) {
   ok = ok && A((void**)&ctx->d_stats, sizeof(DevStats)) == cudaSuccess;
   ok = ok && A((void**)&ctx->d_stats_snap, sizeof(DevStats)) == cudaSuccess;
   ok = ok && A((void**)&ctx->d_spec, (size_t)nb * 2 * sizeof(double)) == cudaSuccess;
-  ok = ok && A((void**)&ctx->d_counters, 64 * sizeof(int)) == cudaSuccess;
+  ok = ok && A((void**)&ctx->d_counters, 72 * sizeof(int)) == cudaSuccess;
   if (!ok) {
     std::string m = cudaGetErrorString(cudaGetLastError());
     free_all(ctx); delete ctx;
@@ -335,6 +338,22 @@ int gm_set_batch(gm_ctx* ctx, int64_t batch_primaries, int64_t queue_records) {
   return GM_OK;
 }
 
+// number of hot/cold pass pairs per generation (gm_set_phase_passes)
+static int phase_pairs_of(const gm_ctx* ctx) {
+  if (ctx->p.metric_kind != 1) return 0;                 // instantiated for the Kerr workloads only
+  if (ctx->phase_pairs >= 0) return ctx->phase_pairs;
+  return ctx->p.thetae_mode != 0 ? 2 : 0;                // a uniform Theta_e has no cold phase
+}
+
+int gm_set_phase_passes(gm_ctx* ctx, int pairs, int k_cold) {
+  if (!ctx) return GM_ERR_PARAM;
+  if (pairs > 8 || k_cold < 1 || k_cold > 1000000) return fail(ctx, GM_ERR_PARAM, "pairs must be <= 8 and k_cold in [1, 1e6]");
+  ctx->phase_pairs = pairs < 0 ? -1 : pairs; ctx->k_cold = k_cold;
+  cudaDeviceSynchronize();
+  free_run_buffers(ctx);
+  return GM_OK;
+}
+
 static int ensure_run_buffers(gm_ctx* ctx, long long n_ids) {
   if (ctx->d_prim_ph) return GM_OK;
   size_t free_b = 0, total_b = 0;
@@ -352,13 +371,20 @@ static int ensure_run_buffers(gm_ctx* ctx, long long n_ids) {
   auto queue_for = [&](long long b) { return ctx->want_queue ? ctx->want_queue : (sc ? 8 * b : (kerr ? b : 1)); };
   long long queue = queue_for(batch);
   // size the batch from the free device memory (at most half of it)
-  auto bytes = [&](long long b, long long q) { return (size_t)(b + 2 * q + (b > q ? b : q)) * sizeof(Photon); };
+  const int pairs = phase_pairs_of(ctx);
+  auto bytes = [&](long long b, long long q) {
+    return (size_t)(b + 2 * q + (pairs > 0 ? 3 : 1) * (b > q ? b : q)) * sizeof(Photon);
+  };
   while (bytes(batch, queue) > free_b / 2 && batch > 1024) { batch >>= 1; queue = queue_for(batch); }
   const long long esc = batch > queue ? batch : queue;
   CK(cudaMalloc((void**)&ctx->d_prim_ph, (size_t)batch * sizeof(Photon)));
   CK(cudaMalloc((void**)&ctx->d_qA, (size_t)queue * sizeof(Photon)));
   CK(cudaMalloc((void**)&ctx->d_qB, (size_t)queue * sizeof(Photon)));
   CK(cudaMalloc((void**)&ctx->d_esc, (size_t)esc * sizeof(Photon)));
+  if (pairs > 0) {
+    CK(cudaMalloc((void**)&ctx->d_parkA, (size_t)esc * sizeof(Photon)));
+    CK(cudaMalloc((void**)&ctx->d_parkB, (size_t)esc * sizeof(Photon)));
+  }
   ctx->batch_primaries = batch; ctx->queue_records = queue; ctx->esc_records = esc;
   return GM_OK;
 }
@@ -370,7 +396,7 @@ static int run_batch(gm_ctx* ctx, long long first, int n, const long long* d_ids
                      Tally tally, DevStats* stats, cudaStream_t st, int* max_queue) {
   int* cnt = ctx->d_counters;       // [0] primaries, [1] work counter, [2] escape queue, [3 + round] queue filled by that round
   const int NCNT = 64, MAXROUND = NCNT - 3;
-  CK(cudaMemsetAsync(cnt, 0, NCNT * sizeof(int), st));
+  CK(cudaMemsetAsync(cnt, 0, 72 * sizeof(int), st));
   TIMED(GM_T_EMIT, st, launch_emit(ctx->P, ctx->Z, ctx->nz, first, n, d_ids, ctx->d_prim_ph, cnt + 0, stats, nullptr, with_root, st));
   const int qcap = (int)ctx->queue_records;
   const Photon* in = ctx->d_prim_ph;
@@ -378,6 +404,12 @@ static int run_batch(gm_ctx* ctx, long long first, int n, const long long* d_ids
   int in_cap = (int)ctx->batch_primaries;
   const int layers = ctx->p.scattering_on ? ctx->p.nsc_max : 0;
   Queue esc{ctx->d_esc, cnt + 2, (int)ctx->esc_records};
+  // automatic schedule: every pass ends with a tail of few long histories, so the passes pay only when a
+  // generation fills the machine many times over (measured: profiles/r01c, break-even near 5e5 primaries)
+  const bool small_batch = ctx->phase_pairs < 0 && n < 500000;
+  const int pairs = (ctx->d_parkA && !small_batch) ? phase_pairs_of(ctx) : 0;
+  Queue nopark{nullptr, cnt + 66, 0};
+  Queue parkA{ctx->d_parkA, cnt + 64, (int)ctx->esc_records}, parkB{ctx->d_parkB, cnt + 65, (int)ctx->esc_records};
   int h_counts[NCNT];
   int mq = 0, round = 0;
   for (;;) {
@@ -385,7 +417,25 @@ static int run_batch(gm_ctx* ctx, long long first, int n, const long long* d_ids
     const int last = round + layers;
     for (; round <= last && round < MAXROUND; round++) {
       Queue out{(round & 1) ? ctx->d_qB : ctx->d_qA, cnt + 3 + round, qcap};
-      TIMED(GM_T_TRACK, st, launch_track(ctx->P, in, in_count, in_cap, cnt + 1, out, esc, tally, stats, trace, ctx->n_sm, st));
+      CK(cudaMemsetAsync(esc.count, 0, sizeof(int), st));
+      if (pairs == 0) {
+        TIMED(GM_T_TRACK, st, launch_track(ctx->P, 0, in, in_count, in_cap, cnt + 1, out, esc, nopark, 0, tally, stats, trace, ctx->n_sm, st));
+      } else {
+        // hot pass (in -> parkA), cold pass (parkA -> parkB), hot pass (parkB -> parkA), ... ; the last cold
+        // pass handles hot plasma in place.  Every queue is fully consumed before it is refilled.
+        const Photon* pin = in; const int* pcount = in_count; int pcap = in_cap;
+        for (int pp = 0; pp < pairs; pp++) {
+          CK(cudaMemsetAsync(parkA.count, 0, sizeof(int), st));
+          TIMED(GM_T_TRACK, st, launch_track(ctx->P, 1, pin, pcount, pcap, cnt + 1, out, esc, parkA, ctx->k_cold, tally, stats, trace, ctx->n_sm, st));
+          if (pp == pairs - 1) {
+            TIMED(GM_T_TRACK, st, launch_track(ctx->P, 0, parkA.buf, parkA.count, parkA.capacity, cnt + 1, out, esc, nopark, 0, tally, stats, trace, ctx->n_sm, st));
+          } else {
+            CK(cudaMemsetAsync(parkB.count, 0, sizeof(int), st));
+            TIMED(GM_T_TRACK, st, launch_track(ctx->P, 2, parkA.buf, parkA.count, parkA.capacity, cnt + 1, out, esc, parkB, 0, tally, stats, trace, ctx->n_sm, st));
+            pin = parkB.buf; pcount = parkB.count; pcap = parkB.capacity;
+          }
+        }
+      }
       TIMED(GM_T_COMPTON, st, launch_compton(ctx->P, out, stats, trace, ctx->n_sm, st));
       TIMED(GM_T_ESCAPE, st, launch_escape(ctx->P, esc, out, tally, stats, trace, ctx->n_sm, st));
       in = out.buf; in_count = out.count; in_cap = qcap;

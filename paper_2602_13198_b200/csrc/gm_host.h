@@ -40,10 +40,12 @@ cudaError_t launch_emit(const DevParams& P, const ZoneArrays& Z, long nz, long l
                         DevStats* stats, gm_emit_rec* emit_out /* or nullptr */, bool with_root,
                         cudaStream_t st);
 // track every photon of `in` (count read from device) until it stops or leaves the grid outwards; scattering
-// events append proto-children (parent state at the event) to `out`, leavers go to `esc` (count reset here)
-cudaError_t launch_track(const DevParams& P, const Photon* in, const int* in_count, int in_capacity,
-                         int* work_counter, Queue out, Queue esc, Tally tally, DevStats* stats, TraceBuf trace,
-                         int n_sm, cudaStream_t st);
+// events append proto-children (parent state at the event) to `out`, leavers go to `esc` (the caller resets
+// esc.count once per generation).  phase 0: everything in place; 1 (hot pass): a lane that was cold for k_cold
+// committed steps is moved to `park`; 2 (cold pass): a lane that meets hot plasma is moved to `park`.
+cudaError_t launch_track(const DevParams& P, int phase, const Photon* in, const int* in_count, int in_capacity,
+                         int* work_counter, Queue out, Queue esc, Queue park, int k_cold, Tally tally, DevStats* stats,
+                         TraceBuf trace, int n_sm, cudaStream_t st);
 // free flight of the leavers to r_max (record) ; a superphoton that re-enters the grid is appended to `ret`
 cudaError_t launch_escape(const DevParams& P, Queue esc, Queue ret, Tally tally, DevStats* stats, TraceBuf trace,
                           int n_sm, cudaStream_t st);

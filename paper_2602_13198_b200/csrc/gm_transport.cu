@@ -16,6 +16,7 @@
 namespace gm {
 
 constexpr int FLAG_ROOT = 1, FLAG_DEAD = 2;
+constexpr int FLAG_ROULETTED = 4;   // the roulette of step `nstep` was already played (record moved between passes)
 
 // ---- block-level stats helper ---------------------------------------------------------------------
 __device__ __forceinline__ void stat_add_n(DevStats* st, int which, unsigned long long v) {
@@ -150,8 +151,22 @@ __global__ void __launch_bounds__(128) emit_kernel(const DevParams P, ZoneArrays
 // lane; stopped lanes are refilled together from a per-warp shared-memory stage that is loaded 32
 // records (5 KB, contiguous) at a time; rare outcomes (record, kill, roulette) sit in out-of-line
 // functions so that the hot loop stays small enough for the instruction cache.
+//
+// Phase passes (PHASE template argument).  Absorption (Eq. 16-20) is evaluated only in
+// plasma with Theta_e >= thetae_min -- in the torus workloads 13 % of the in-grid steps, mostly at the start of a
+// history (superphotons are emitted and scattered where the plasma is hot).  With young and old histories mixed
+// in one warp that block runs at 4 of 32 lanes in nearly every iteration.  So a generation is tracked in passes:
+//   PHASE_HOT   a lane whose last `k_cold` committed steps were all cold stores its state to the `park` queue;
+//   PHASE_COLD  a lane that meets hot plasma stores its start-of-step state to `park` (the step is redone by
+//               the next hot pass; nothing of the absorption block is executed in this pass);
+//   PHASE_MIXED everything in place (the last pass of a generation, and every pass of the flat workloads).
+// A history is a pure function of its record (counter-based RNG), so the passes change no result.
 // =====================================================================================================
-constexpr int TRACK_THREADS = 128;
+constexpr int PHASE_MIXED = 0, PHASE_HOT = 1, PHASE_COLD = 2;
+#ifndef GM_TRACK_THREADS
+#define GM_TRACK_THREADS 128
+#endif
+constexpr int TRACK_THREADS = GM_TRACK_THREADS;
 constexpr int TRACK_WARPS = TRACK_THREADS / 32;
 constexpr int PH_U4 = sizeof(Photon) / 16;          // 10 x 16 B per record
 
@@ -277,10 +292,15 @@ __device__ __forceinline__ bool stop_tests(const DevParams& P, Lane& L, const Ta
 #define GM_TRACK_MINBLOCKS 3
 #endif
 
-template <bool KERR, bool THREED>
+template <bool KERR, bool THREED, int PHASE>
+#ifdef GM_TRACK_MAXNREG
+__global__ void __maxnreg__(GM_TRACK_MAXNREG)
+#else
 __global__ void __launch_bounds__(TRACK_THREADS, GM_TRACK_MINBLOCKS)
+#endif
 track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in, const int* __restrict__ in_count, int in_capacity,
-             int* work_counter, Queue out, Queue esc, Tally tally, DevStats* stats, TraceBuf trace) {
+             int* work_counter, Queue out, Queue esc, Queue park, int k_cold, Tally tally, DevStats* stats,
+             TraceBuf trace) {
   __shared__ uint4 s_stage[TRACK_WARPS][32 * PH_U4];      // 4 x 5 KB: next 32 records of each warp
   const int n_in = min(*in_count, in_capacity);
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -291,9 +311,11 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
   L.id0 = L.id1 = L.id2 = L.nstep = L.jscat = 0u; L.nsc = 0; L.root = -1; L.flags = 0;
 #pragma unroll
   for (int m = 0; m < 4; m++) { L.x[m] = 0.0; L.k[m] = 0.0; L.a[m] = 0.0; }
-  bool have = false, want_scat = false;
+  bool have = false;
+  int ncold = 0;                        // PHASE_HOT: consecutive committed cold steps of this lane
   int mode = 0;                         // 0 normal step, 1 partial push to a scattering event, 2 redo full step
   double dl = 0.0, ux = 0.0, ev_f = 0.0, ev_b = 1.0, ev_tau = 0.0;
+  int ev_it = 0;                        // PHASE_COLD: Verlet iterations counted for the attempt that found the event
   int st_next = 0, st_avail = 0;        // staged records [st_next, st_avail); warp-uniform
   bool exhausted = false;               // warp-uniform
   unsigned long long c_steps = 0, c_viters = 0;
@@ -324,8 +346,7 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
         if (!have && rank < left) {
           lane_load(L, reinterpret_cast<const Photon*>(stage) + st_next + rank);
           if (!(L.flags & FLAG_DEAD)) {
-            have = true; mode = 0;
-            want_scat = P.scattering_on != 0 && L.nsc < P.nsc_max;
+            have = true; mode = 0; ncold = 0;
           }
         }
         st_next += min(__popc(need), left);
@@ -345,14 +366,16 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
       }
       double ur;
       uniform_pair(P, TAG_STEP, L.id0, L.id1, L.id2, L.nstep, ux, ur);
-      if (L.w < P.w_min) {
+      if (L.w < P.w_min && !(L.flags & FLAG_ROULETTED)) {
         const Lane T = L;
         L.w = roulette(P, T, ur, stats, trace);
         if (L.w < 0.0) { have = false; continue; }
+        L.flags |= FLAG_ROULETTED;                        // cleared when the step is committed
       }
       dl = step_size(P, L.x, L.k);
     }
     const double dl_eff = (mode == 1) ? ev_f * dl : dl;
+    const bool want_scat = P.scattering_on != 0 && L.nsc < P.nsc_max;   // cheaper than a flag kept across the loop
     double x1[4], k1[4], a1[4];
     Geom G;
     bool capped;
@@ -364,9 +387,25 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
     const int it = push_wavevector<KERR>(P, L.k, L.a, dl_eff, x1, k1, a1, G, capped);
     Plasma S;
     double na1 = 0.0, ns1 = 0.0, b1 = 1.0;
+    bool hot = false;
     if (inplasma) {
       plasma_from_prim(P, G, pr, S);
-      opacities(P, k1, G, S, L.nsc, want_scat, na1, ns1, b1);
+      hot = S.thetae >= P.thetae_min && S.B > 0.0;         // the condition under which opacities() absorbs
+      if (PHASE == PHASE_COLD) {
+        if (hot) {                                         // park the start-of-step state for the next hot pass
+          const int slot = atomicAdd(park.count, 1);
+          if (slot < park.capacity) lane_store(L, park.buf + slot);
+          if (mode != 0) {                                 // the attempt of this step is redone: uncount it
+            c_viters -= (unsigned long long)abs(ev_it);
+            if (ev_it < 0) atomicAdd(&stats->n[SN_VCAPPED], ~0ull);
+          }
+          have = false; mode = 0;
+          continue;
+        }
+        opacities<false>(P, k1, G, S, L.nsc, want_scat, na1, ns1, b1);
+      } else {
+        opacities<true>(P, k1, G, S, L.nsc, want_scat, na1, ns1, b1);
+      }
     }
 
     if (mode == 1) {
@@ -394,6 +433,7 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
       L.jscat++;
       L.nua_a = na1; L.nua_s = ns1; L.bias = b1;
       L.nstep++; c_steps++;
+      L.flags &= ~FLAG_ROULETTED;
       mode = 0;
       if (!(L.w > 0.0)) {                                    // analog limit b = 1
         const Lane T = L;
@@ -410,11 +450,14 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
         const double tau_s = 0.5 * (L.nua_s + ns1) * P.Cfac * dl;      // Eq. 25
         const double bt = 0.5 * (L.bias + b1) * tau_s;                 // G19
         // x_r = -ln(1-u) >= u: the logarithm is needed only when b tau_s exceeds u
-        if (bt > ux) {
-          const double b = 0.5 * (L.bias + b1);
+        const double b = 0.5 * (L.bias + b1);
+        // w/b >= w_min is the other condition of the event (G21): a weight below half of w_min b cannot meet it,
+        // whatever the rounding of the division, and needs no logarithm
+        if (bt > ux && L.w > 0.5 * P.w_min * b) {
           const double xr = -log(1.0 - ux);
           if (bt > xr && L.w / b >= P.w_min) {
             mode = 1; ev_f = xr / bt; ev_b = b; ev_tau = tau_a;
+            if (PHASE == PHASE_COLD) ev_it = capped ? -it : it;
             continue;
           }
         }
@@ -430,7 +473,16 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
     for (int m = 0; m < 4; m++) { L.x[m] = x1[m]; L.k[m] = k1[m]; L.a[m] = a1[m]; }
     L.nua_a = na1; L.nua_s = ns1; L.bias = b1;
     L.nstep++; c_steps++;
+    L.flags &= ~FLAG_ROULETTED;
     mode = 0;
+    if (PHASE == PHASE_HOT) {
+      ncold = hot ? 0 : ncold + 1;
+      if (ncold >= k_cold && L.x[1] < P.x1hi) {            // cold for k_cold steps: continue in the cold pass
+        const int slot = atomicAdd(park.count, 1);
+        if (slot < park.capacity) lane_store(L, park.buf + slot);
+        have = false;
+      }
+    }
   }
   // flush thread-local counters
   for (int o = 16; o > 0; o >>= 1) {
@@ -773,15 +825,29 @@ cudaError_t launch_emit(const DevParams& P, const ZoneArrays& Z, long nz, long l
   return cudaGetLastError();
 }
 
-cudaError_t launch_track(const DevParams& P, const Photon* in, const int* in_count, int in_capacity,
-                         int* work_counter, Queue out, Queue esc, Tally tally, DevStats* stats, TraceBuf trace,
-                         int n_sm, cudaStream_t st) {
+cudaError_t launch_track(const DevParams& P, int phase, const Photon* in, const int* in_count, int in_capacity,
+                         int* work_counter, Queue out, Queue esc, Queue park, int k_cold, Tally tally, DevStats* stats,
+                         TraceBuf trace, int n_sm, cudaStream_t st) {
   cudaError_t e = cudaMemsetAsync(work_counter, 0, sizeof(int), st);
   if (e != cudaSuccess) return e;
-  if ((e = cudaMemsetAsync(esc.count, 0, sizeof(int), st)) != cudaSuccess) return e;
   const int grid = n_sm * GM_TRACK_MINBLOCKS;
-  GM_DISPATCH(track_kernel, grid, TRACK_THREADS, st, P, in, in_count, in_capacity, work_counter, out, esc, tally, stats,
-              trace);
+  const bool kerr = P.metric_kind == 1, td = P.n3 > 1;
+#define GM_TRACK_ARGS P, in, in_count, in_capacity, work_counter, out, esc, park, k_cold, tally, stats, trace
+  if (phase == PHASE_MIXED) {
+    if (kerr && td) track_kernel<true, true, PHASE_MIXED><<<grid, TRACK_THREADS, 0, st>>>(GM_TRACK_ARGS);
+    else if (kerr) track_kernel<true, false, PHASE_MIXED><<<grid, TRACK_THREADS, 0, st>>>(GM_TRACK_ARGS);
+    else if (td) track_kernel<false, true, PHASE_MIXED><<<grid, TRACK_THREADS, 0, st>>>(GM_TRACK_ARGS);
+    else track_kernel<false, false, PHASE_MIXED><<<grid, TRACK_THREADS, 0, st>>>(GM_TRACK_ARGS);
+  } else if (!kerr) {
+    return cudaErrorInvalidValue;        // phase passes are instantiated for the Kerr workloads only
+  } else if (phase == PHASE_HOT) {
+    if (td) track_kernel<true, true, PHASE_HOT><<<grid, TRACK_THREADS, 0, st>>>(GM_TRACK_ARGS);
+    else track_kernel<true, false, PHASE_HOT><<<grid, TRACK_THREADS, 0, st>>>(GM_TRACK_ARGS);
+  } else {
+    if (td) track_kernel<true, true, PHASE_COLD><<<grid, TRACK_THREADS, 0, st>>>(GM_TRACK_ARGS);
+    else track_kernel<true, false, PHASE_COLD><<<grid, TRACK_THREADS, 0, st>>>(GM_TRACK_ARGS);
+  }
+#undef GM_TRACK_ARGS
   return cudaGetLastError();
 }
 

@@ -340,6 +340,45 @@ def test_config4_analog_scattering_small(gm):
     _compare_traces(o, g, ids, fork_budget=5e-3)
 
 
+@pytest.mark.parametrize("cfg,pairs,k_cold", [(2, 1, 1), (2, 2, 4), (2, 3, 2), (3, 2, 3), (4, 2, 1)])
+def test_hot_cold_phase_passes_change_no_history(gm, cfg, pairs, k_cold):
+    """Tracker schedule (gm_set_phase_passes): a history is a pure function of its record, so
+    handing superphotons between hot and cold passes must leave every counter and every bin count unchanged
+    (sums differ only by the order of the fp64 atomics).  The forced schedule is also compared with the oracle."""
+    if cfg == 2:
+        p, prim = wl.config2(Ns=2e4)
+    elif cfg == 3:
+        p, prim = wl.config3(Ns=1e4, n1=48, n2=32, n3=32)
+    else:
+        p, prim = wl.config4(Ns=5e3)
+    res = []
+    for pr_ in (0, pairs):
+        g = gm.GPUMonty(p)
+        g.set_phase_passes(pr_, k_cold)
+        g.set_grid(prim)
+        g.prepare()
+        g.run()
+        res.append((g.stats(), g.tally(), g))
+    s0, s1 = res[0][0], res[1][0]
+    for k in s0:
+        if k.startswith("n_"):
+            assert s0[k] == s1[k], (k, s0[k], s1[k])
+        else:
+            assert s1[k] == pytest.approx(s0[k], rel=1e-11, abs=1e-300), k
+    (A0, Q0, W0, n0), (A1, Q1, W1, n1) = res[0][1], res[1][1]
+    assert np.array_equal(n0, n1)
+    assert np.allclose(A0, A1, rtol=1e-11, atol=0) and np.allclose(W0, W1, rtol=1e-11, atol=0)
+    ids = np.arange(0, res[1][2].n_primaries, 13)
+    t0, t1 = res[0][2].trace(ids), res[1][2].trace(ids)
+    for f in ("fate", "nstep", "inu", "ith", "jscat", "fam_nspawn"):
+        assert np.array_equal(t0[f], t1[f]), f
+    assert np.array_equal(t0["w"], t1["w"]) and np.array_equal(t0["x"], t1["x"])
+    from oracle_binding import Oracle
+    o = Oracle(p, prim)
+    o.prepare(); o.run()
+    _compare_stats(o, res[1][2], rel=5e-3)
+
+
 @pytest.mark.parametrize("scattering", [0, 1])
 def test_superphotons_reentering_the_grid_from_free_flight(gm, scattering):
     """Degenerate case of the escape split: a Kerr grid that ends at r = 2.2, inside the
