@@ -291,12 +291,15 @@ __device__ __forceinline__ bool stop_tests(const DevParams& P, Lane& L, const Ta
 #ifndef GM_TRACK_MINBLOCKS
 #define GM_TRACK_MINBLOCKS 3
 #endif
+#ifndef GM_COLD_MINBLOCKS
+#define GM_COLD_MINBLOCKS GM_TRACK_MINBLOCKS
+#endif
 
 template <bool KERR, bool THREED, int PHASE>
 #ifdef GM_TRACK_MAXNREG
 __global__ void __maxnreg__(GM_TRACK_MAXNREG)
 #else
-__global__ void __launch_bounds__(TRACK_THREADS, GM_TRACK_MINBLOCKS)
+__global__ void __launch_bounds__(TRACK_THREADS, PHASE == 2 ? GM_COLD_MINBLOCKS : GM_TRACK_MINBLOCKS)
 #endif
 track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in, const int* __restrict__ in_count, int in_capacity,
              int* work_counter, Queue out, Queue esc, Queue park, int k_cold, Tally tally, DevStats* stats,
@@ -830,7 +833,7 @@ cudaError_t launch_track(const DevParams& P, int phase, const Photon* in, const 
                          TraceBuf trace, int n_sm, cudaStream_t st) {
   cudaError_t e = cudaMemsetAsync(work_counter, 0, sizeof(int), st);
   if (e != cudaSuccess) return e;
-  const int grid = n_sm * GM_TRACK_MINBLOCKS;
+  const int grid = n_sm * (phase == PHASE_COLD ? GM_COLD_MINBLOCKS : GM_TRACK_MINBLOCKS);
   const bool kerr = P.metric_kind == 1, td = P.n3 > 1;
 #define GM_TRACK_ARGS P, in, in_count, in_capacity, work_counter, out, esc, park, k_cold, tally, stats, trace
   if (phase == PHASE_MIXED) {
