@@ -36,11 +36,14 @@ from paper_2602_13198_b200.shard import rank_seed, reduce_tally  # noqa: E402
 METRIC = "superphotons/s tracked (incl. scattering)"
 UNIT = "superphotons/s"
 # algorithmic FP64 flop per geodesic step (dadd + dmul + 2 dfma predicated-on thread
-# instructions of the kernel divided by the steps it committed, counted with ncu on each workload class --
-# profiles/r01b_flop_per_step.md -- and then frozen).  "track": in-grid step of track_kernel; "escape":
-# free-flight step of escape_kernel.
-FLOP_PER_STEP = {"flat": {"track": 853.0, "escape": 223.0}, "kerr": {"track": 877.0, "escape": 434.0},
-                 "kerr3d": {"track": 877.0, "escape": 434.0}}
+# instructions of the kernel divided by the steps it committed, counted with ncu on each workload class with the
+# single mixed tracker pass, so that no redone step is counted -- profiles/r01d_flop_per_step.md -- and then
+# frozen).  "track": in-grid step of track_kernel; "escape": free-flight step of escape_kernel.
+FLOP_PER_STEP = {"flat": {"track": 676.3, "escape": 207.9}, "kerr": {"track": 693.2, "escape": 367.1},
+                 "kerr3d": {"track": 795.1, "escape": 367.1}}
+# dram__bytes_read.sum + dram__bytes_write.sum of the dominant launch (cold tracker pass over 1.09e6 primaries,
+# cfg2 at Ns=3e6) from the ncu --set full capture of profiles/r01c_phase_passes.md; quoted for cfg2 only
+TRAFFIC_BYTES_PER_LAUNCH = {2: 86.9e6 + 78.5e6}
 WORKLOAD_NAMES = {0: "cfg0 thin synchrotron sphere 32x16, Ns=1e5", 1: "cfg1 scattering sphere 32x16, Ns=1e6",
                   2: "cfg2 Kerr FM torus 256x256, Ns=1e7", 3: "cfg3 3-D perturbed torus 192x128x128, Ns=1e7",
                   4: "cfg4 Kerr torus x1e3 density (analog scattering), Ns=1e6"}
@@ -255,7 +258,7 @@ def main():
             "gpu_launches": int(launches),
             "clocks": clk,
             "roofline": {"bound": "alu", "kernel": "track_kernel", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                         "frac": achieved / peak, "traffic": None,
+                         "frac": achieved / peak, "traffic": TRAFFIC_BYTES_PER_LAUNCH.get(args.config),
                          "peak_source": "DFMA-chain microbenchmark run in this process (gm_fp64_peak); nominal 2*64*148*1.965 GHz = 37.2",
                          "flop_per_step": FLOP_PER_STEP[kind]["track"], "track_ms_per_step": track_ms_per_step,
                          "escape_kernel": {"achieved": esc_tflops, "frac": esc_tflops / peak, "ms_per_step": esc_ms,
