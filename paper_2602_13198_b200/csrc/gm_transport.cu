@@ -169,6 +169,14 @@ constexpr int PHASE_MIXED = 0, PHASE_HOT = 1, PHASE_COLD = 2;
 constexpr int TRACK_THREADS = GM_TRACK_THREADS;
 constexpr int TRACK_WARPS = TRACK_THREADS / 32;
 constexpr int PH_U4 = sizeof(Photon) / 16;          // 10 x 16 B per record
+// The 2-D gather (4 zone records) is staged through shared memory with asynchronous copies; the 3-D one (8 records,
+// 16 KB of slots per warp) is not: its slots would leave no L1 for the line sharing between neighbouring records,
+// and measured slower either way (profiles/r01e).  Refill stage: 32 records (5 KB) per warp.
+__host__ __device__ constexpr bool track_staged_gather(bool threed) { return !threed; }
+__host__ __device__ constexpr int track_stage_records(bool) { return 32; }
+__host__ __device__ constexpr int track_smem_bytes(bool threed) {
+  return TRACK_WARPS * (track_stage_records(threed) * PH_U4 + (track_staged_gather(threed) ? 4 * 4 * 32 : 0)) * 16;
+}
 
 struct Lane {                                       // registers of the current superphoton
   double x[4], k[4], a[4], w, nua_a, nua_s, bias;
@@ -304,11 +312,16 @@ __global__ void __launch_bounds__(TRACK_THREADS, PHASE == 2 ? GM_COLD_MINBLOCKS 
 track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in, const int* __restrict__ in_count, int in_capacity,
              int* work_counter, Queue out, Queue esc, Queue park, int k_cold, Tally tally, DevStats* stats,
              TraceBuf trace) {
-  __shared__ uint4 s_stage[TRACK_WARPS][32 * PH_U4];      // 4 x 5 KB: next 32 records of each warp
+  // dynamic shared memory: per warp the next STAGE_REC records (refill stage) and the gather slots of its lanes
+  extern __shared__ uint4 s_dyn[];
+  constexpr int STAGE_REC = track_stage_records(THREED);
+  constexpr bool STAGED = track_staged_gather(THREED);
+  constexpr int GATHER_U4 = STAGED ? 4 * 4 * 32 : 0;      // 16-byte slots per warp: records x 4 parts x 32 lanes
   const int n_in = min(*in_count, in_capacity);
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const unsigned lt_mask = (1u << lane) - 1u;
-  uint4* stage = s_stage[wid];
+  uint4* stage = s_dyn + wid * (STAGE_REC * PH_U4);
+  uint4* sg = s_dyn + TRACK_WARPS * (STAGE_REC * PH_U4) + wid * GATHER_U4 + lane;
   Lane L;
   L.w = 0.0; L.nua_a = 0.0; L.nua_s = 0.0; L.bias = 1.0;
   L.id0 = L.id1 = L.id2 = L.nstep = L.jscat = 0u; L.nsc = 0; L.root = -1; L.flags = 0;
@@ -331,9 +344,9 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
     if (need) {
       if (st_next == st_avail && !exhausted) {
         int base = 0;
-        if (lane == 0) base = atomicAdd(work_counter, 32);
+        if (lane == 0) base = atomicAdd(work_counter, STAGE_REC);
         base = __shfl_sync(0xffffffffu, base, 0);
-        const int cnt = min(32, n_in - base);
+        const int cnt = min(STAGE_REC, n_in - base);
         if (cnt <= 0) {
           exhausted = true;
         } else {
@@ -386,8 +399,17 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
     // the gather needs only the position: issue it before the metric work of the push so that the loads fly
     // while the FP64 pipe is busy (S8)
     double pr[8];
-    const bool inplasma = interp_prim<THREED>(P, x1, pr) && pr[0] > 0.0;
-    const int it = push_wavevector<KERR>(P, L.k, L.a, dl_eff, x1, k1, a1, G, capped);
+    bool inplasma = false;
+    int it;
+    if (STAGED) {
+      GatherW gw;
+      const bool ingrid = gather_issue<THREED>(P, x1, sg, gw);     // asynchronous copies fly during the push
+      it = push_wavevector<KERR>(P, L.k, L.a, dl_eff, x1, k1, a1, G, capped);
+      if (ingrid) { gather_finish<THREED>(sg, gw, pr); inplasma = pr[0] > 0.0; }
+    } else {
+      inplasma = interp_prim<THREED>(P, x1, pr) && pr[0] > 0.0;
+      it = push_wavevector<KERR>(P, L.k, L.a, dl_eff, x1, k1, a1, G, capped);
+    }
     Plasma S;
     double na1 = 0.0, ns1 = 0.0, b1 = 1.0;
     bool hot = false;
@@ -836,19 +858,29 @@ cudaError_t launch_track(const DevParams& P, int phase, const Photon* in, const 
   const int grid = n_sm * (phase == PHASE_COLD ? GM_COLD_MINBLOCKS : GM_TRACK_MINBLOCKS);
   const bool kerr = P.metric_kind == 1, td = P.n3 > 1;
 #define GM_TRACK_ARGS P, in, in_count, in_capacity, work_counter, out, esc, park, k_cold, tally, stats, trace
+  const int smem = track_smem_bytes(td);
+  static bool attr_set = false;
+  if (!attr_set) {                       // > 48 KB of dynamic shared memory needs the opt-in, once per kernel
+#define GM_OPTIN(K, T, PH) cudaFuncSetAttribute(track_kernel<K, T, PH>, cudaFuncAttributeMaxDynamicSharedMemorySize, track_smem_bytes(T))
+    GM_OPTIN(true, true, PHASE_MIXED); GM_OPTIN(true, false, PHASE_MIXED); GM_OPTIN(false, true, PHASE_MIXED);
+    GM_OPTIN(false, false, PHASE_MIXED); GM_OPTIN(true, true, PHASE_HOT); GM_OPTIN(true, false, PHASE_HOT);
+    GM_OPTIN(true, true, PHASE_COLD); GM_OPTIN(true, false, PHASE_COLD);
+#undef GM_OPTIN
+    attr_set = true;
+  }
   if (phase == PHASE_MIXED) {
-    if (kerr && td) track_kernel<true, true, PHASE_MIXED><<<grid, TRACK_THREADS, 0, st>>>(GM_TRACK_ARGS);
-    else if (kerr) track_kernel<true, false, PHASE_MIXED><<<grid, TRACK_THREADS, 0, st>>>(GM_TRACK_ARGS);
-    else if (td) track_kernel<false, true, PHASE_MIXED><<<grid, TRACK_THREADS, 0, st>>>(GM_TRACK_ARGS);
-    else track_kernel<false, false, PHASE_MIXED><<<grid, TRACK_THREADS, 0, st>>>(GM_TRACK_ARGS);
+    if (kerr && td) track_kernel<true, true, PHASE_MIXED><<<grid, TRACK_THREADS, smem, st>>>(GM_TRACK_ARGS);
+    else if (kerr) track_kernel<true, false, PHASE_MIXED><<<grid, TRACK_THREADS, smem, st>>>(GM_TRACK_ARGS);
+    else if (td) track_kernel<false, true, PHASE_MIXED><<<grid, TRACK_THREADS, smem, st>>>(GM_TRACK_ARGS);
+    else track_kernel<false, false, PHASE_MIXED><<<grid, TRACK_THREADS, smem, st>>>(GM_TRACK_ARGS);
   } else if (!kerr) {
     return cudaErrorInvalidValue;        // phase passes are instantiated for the Kerr workloads only
   } else if (phase == PHASE_HOT) {
-    if (td) track_kernel<true, true, PHASE_HOT><<<grid, TRACK_THREADS, 0, st>>>(GM_TRACK_ARGS);
-    else track_kernel<true, false, PHASE_HOT><<<grid, TRACK_THREADS, 0, st>>>(GM_TRACK_ARGS);
+    if (td) track_kernel<true, true, PHASE_HOT><<<grid, TRACK_THREADS, smem, st>>>(GM_TRACK_ARGS);
+    else track_kernel<true, false, PHASE_HOT><<<grid, TRACK_THREADS, smem, st>>>(GM_TRACK_ARGS);
   } else {
-    if (td) track_kernel<true, true, PHASE_COLD><<<grid, TRACK_THREADS, 0, st>>>(GM_TRACK_ARGS);
-    else track_kernel<true, false, PHASE_COLD><<<grid, TRACK_THREADS, 0, st>>>(GM_TRACK_ARGS);
+    if (td) track_kernel<true, true, PHASE_COLD><<<grid, TRACK_THREADS, smem, st>>>(GM_TRACK_ARGS);
+    else track_kernel<true, false, PHASE_COLD><<<grid, TRACK_THREADS, smem, st>>>(GM_TRACK_ARGS);
   }
 #undef GM_TRACK_ARGS
   return cudaGetLastError();
