@@ -5,6 +5,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -27,7 +28,9 @@ struct gm_ctx {
   int* d_counters = nullptr;         // [0] primaries count, [1] queue A count, [2] queue B count, [3] work counter
   Photon *d_prim_ph = nullptr, *d_qA = nullptr, *d_qB = nullptr, *d_esc = nullptr;
   Photon *d_parkA = nullptr, *d_parkB = nullptr;   // hot/cold pass hand-over queues (esc_records each)
-  int phase_pairs = -1, k_cold = 4;                // -1: automatic (2 for Kerr with a temperature model, else 0)
+  int phase_pairs = -1, k_cold = 4;                // -1: automatic (decided by a pilot batch, see gm_run)
+  int auto_pairs = -1;                             // the pilot's decision (-1: not taken yet)
+  double pilot_cold_fraction = -1.0;
   long long esc_records = 0;
   long long batch_primaries = 0, queue_records = 0;   // allocated sizes
   long long want_batch = 0, want_queue = 0;
@@ -294,6 +297,7 @@ int gm_prepare(gm_ctx* ctx, void* cuda_stream, int64_t* n_primaries_out) {
   if (bad) return fail(ctx, GM_ERR_GRID, "non-finite value in the fluid grid");
   ctx->n_primaries = total;
   ctx->prepared = true;
+  ctx->auto_pairs = -1;
   int r = gm_reset_tally(ctx);
   if (r != GM_OK) return r;
   if (n_primaries_out) *n_primaries_out = total;
@@ -342,13 +346,14 @@ int gm_set_batch(gm_ctx* ctx, int64_t batch_primaries, int64_t queue_records) {
 static int phase_pairs_of(const gm_ctx* ctx) {
   if (ctx->p.metric_kind != 1) return 0;                 // instantiated for the Kerr workloads only
   if (ctx->phase_pairs >= 0) return ctx->phase_pairs;
-  return ctx->p.thetae_mode != 0 ? 2 : 0;                // a uniform Theta_e has no cold phase
+  if (ctx->p.thetae_mode == 0) return 0;                 // a uniform Theta_e has no cold phase
+  return ctx->auto_pairs >= 0 ? ctx->auto_pairs : 2;
 }
 
 int gm_set_phase_passes(gm_ctx* ctx, int pairs, int k_cold) {
   if (!ctx) return GM_ERR_PARAM;
   if (pairs > 8 || k_cold < 1 || k_cold > 1000000) return fail(ctx, GM_ERR_PARAM, "pairs must be <= 8 and k_cold in [1, 1e6]");
-  ctx->phase_pairs = pairs < 0 ? -1 : pairs; ctx->k_cold = k_cold;
+  ctx->phase_pairs = pairs < 0 ? -1 : pairs; ctx->k_cold = k_cold; ctx->auto_pairs = -1;
   cudaDeviceSynchronize();
   free_run_buffers(ctx);
   return GM_OK;
@@ -406,8 +411,14 @@ static int run_batch(gm_ctx* ctx, long long first, int n, const long long* d_ids
   Queue esc{ctx->d_esc, cnt + 2, (int)ctx->esc_records};
   // automatic schedule: every pass ends with a tail of few long histories, so the passes pay only when a
   // generation fills the machine many times over (measured: profiles/r01c, break-even near 5e5 primaries)
-  const bool small_batch = ctx->phase_pairs < 0 && n < 500000;
-  const int pairs = (ctx->d_parkA && !small_batch) ? phase_pairs_of(ctx) : 0;
+  const bool small_batch = ctx->phase_pairs < 0 && n < (ctx->auto_pairs < 0 ? 1000000 : 500000);
+  int pairs = (ctx->d_parkA && !small_batch) ? phase_pairs_of(ctx) : 0;
+  // Automatic schedule, decided once per gm_prepare on the first batch of >= 1e6 primaries: the passes pay when the
+  // superphotons outlive the hot plasma they start in (configs 2-3: 0.47-0.61 of the primaries are handed over by
+  // the first hot pass) and cost when most histories end there (config 4, optically thick with analog
+  // scattering: 0.24-0.27; profiles/r01e).  The first hot pass is run, its hand-over count read back, and the
+  // generation continues with either schedule.
+  bool deciding = ctx->phase_pairs < 0 && ctx->auto_pairs < 0 && pairs > 0 && n >= 1000000;
   Queue nopark{nullptr, cnt + 66, 0};
   Queue parkA{ctx->d_parkA, cnt + 64, (int)ctx->esc_records}, parkB{ctx->d_parkB, cnt + 65, (int)ctx->esc_records};
   int h_counts[NCNT];
@@ -427,7 +438,19 @@ static int run_batch(gm_ctx* ctx, long long first, int n, const long long* d_ids
         for (int pp = 0; pp < pairs; pp++) {
           CK(cudaMemsetAsync(parkA.count, 0, sizeof(int), st));
           TIMED(GM_T_TRACK, st, launch_track(ctx->P, 1, pin, pcount, pcap, cnt + 1, out, esc, parkA, ctx->k_cold, tally, stats, trace, ctx->n_sm, st));
-          if (pp == pairs - 1) {
+          if (deciding) {
+            int parked = 0;
+            CK(cudaMemcpyAsync(&parked, parkA.count, sizeof(int), cudaMemcpyDeviceToHost, st));
+            CK(cudaStreamSynchronize(st));
+            ctx->pilot_cold_fraction = (double)parked / (double)n;
+            ctx->auto_pairs = ctx->pilot_cold_fraction >= 0.35 ? 2 : 0;
+            if (getenv("GPUMONTY_B200_DEBUG"))
+              fprintf(stderr, "[gpumonty_b200] %.3f of the primaries leave the first hot pass alive -> %d pass pairs\n",
+                      ctx->pilot_cold_fraction, ctx->auto_pairs);
+            deciding = false;
+            if (ctx->auto_pairs == 0) pairs = 1;           // finish this generation with the mixed pass, then none
+          }
+          if (pp >= pairs - 1) {
             TIMED(GM_T_TRACK, st, launch_track(ctx->P, 0, parkA.buf, parkA.count, parkA.capacity, cnt + 1, out, esc, nopark, 0, tally, stats, trace, ctx->n_sm, st));
           } else {
             CK(cudaMemsetAsync(parkB.count, 0, sizeof(int), st));
@@ -435,6 +458,7 @@ static int run_batch(gm_ctx* ctx, long long first, int n, const long long* d_ids
             pin = parkB.buf; pcount = parkB.count; pcap = parkB.capacity;
           }
         }
+        if (ctx->phase_pairs < 0 && ctx->auto_pairs == 0) pairs = 0;
       }
       TIMED(GM_T_COMPTON, st, launch_compton(ctx->P, out, stats, trace, ctx->n_sm, st));
       TIMED(GM_T_ESCAPE, st, launch_escape(ctx->P, esc, out, tally, stats, trace, ctx->n_sm, st));
