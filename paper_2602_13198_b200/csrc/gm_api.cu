@@ -461,7 +461,7 @@ static int run_batch(gm_ctx* ctx, long long first, int n, const long long* d_ids
         if (ctx->phase_pairs < 0 && ctx->auto_pairs == 0) pairs = 0;
       }
       TIMED(GM_T_COMPTON, st, launch_compton(ctx->P, out, stats, trace, ctx->n_sm, st));
-      TIMED(GM_T_ESCAPE, st, launch_escape(ctx->P, esc, out, tally, stats, trace, ctx->n_sm, st));
+      TIMED(GM_T_ESCAPE, st, launch_escape(ctx->P, esc, cnt + 1, out, tally, stats, trace, ctx->n_sm, st));
       in = out.buf; in_count = out.count; in_cap = qcap;
     }
     CK(cudaMemcpyAsync(h_counts, cnt, NCNT * sizeof(int), cudaMemcpyDeviceToHost, st));

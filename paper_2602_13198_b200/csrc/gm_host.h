@@ -47,8 +47,8 @@ cudaError_t launch_track(const DevParams& P, int phase, const Photon* in, const 
                          int* work_counter, Queue out, Queue esc, Queue park, int k_cold, Tally tally, DevStats* stats,
                          TraceBuf trace, int n_sm, cudaStream_t st);
 // free flight of the leavers to r_max (record) ; a superphoton that re-enters the grid is appended to `ret`
-cudaError_t launch_escape(const DevParams& P, Queue esc, Queue ret, Tally tally, DevStats* stats, TraceBuf trace,
-                          int n_sm, cudaStream_t st);
+cudaError_t launch_escape(const DevParams& P, Queue esc, int* work_counter, Queue ret, Tally tally, DevStats* stats,
+                          TraceBuf trace, int n_sm, cudaStream_t st);
 // turn the proto-children of `q` into scattered superphotons in place (one Compton event each)
 cudaError_t launch_compton(const DevParams& P, Queue q, DevStats* stats, TraceBuf trace, int n_sm,
                            cudaStream_t st);

@@ -530,38 +530,79 @@ template <bool KERR>
 #define GM_ESC_MINBLOCKS 4
 #endif
 __global__ void __launch_bounds__(128, GM_ESC_MINBLOCKS)
-escape_kernel(const __grid_constant__ DevParams P, Queue esc, Queue ret, Tally tally, DevStats* stats, TraceBuf trace) {
+escape_kernel(const __grid_constant__ DevParams P, Queue esc, int* work_counter, Queue ret, Tally tally, DevStats* stats,
+              TraceBuf trace) {
+  // persistent, refilled like the tracker: the 32 lanes of a warp step together, stopped lanes take the next
+  // records from a shared-memory stage that is loaded 32 records at a time (coalesced, ahead of their use)
+  __shared__ uint4 s_stage[4][32 * PH_U4];
   const int n = min(*esc.count, esc.capacity);
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  const unsigned lt_mask = (1u << lane) - 1u;
+  uint4* stage = s_stage[wid];
   unsigned long long c_steps = 0, c_viters = 0, c_capped = 0;
-  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
-    Lane L;
-    lane_load(L, esc.buf + i);
-    for (;;) {
-      if (stop_tests<KERR>(P, L, tally, stats, trace)) break;
-      if (L.x[1] < P.x1hi) {                                 // back inside the grid
-        L.nua_a = 0.0; L.nua_s = 0.0; L.bias = 1.0;          // opacities at a vacuum point
-        const int slot = atomicAdd(ret.count, 1);
-        if (slot < ret.capacity) lane_store(L, ret.buf + slot);
-        atomicAdd(&stats->n[SN_REENTER], 1ull);
+  Lane L;
+  L.w = 0.0; L.nua_a = 0.0; L.nua_s = 0.0; L.bias = 1.0;
+  L.id0 = L.id1 = L.id2 = L.nstep = L.jscat = 0u; L.nsc = 0; L.root = -1; L.flags = 0;
+#pragma unroll
+  for (int m = 0; m < 4; m++) { L.x[m] = 0.0; L.k[m] = 0.0; L.a[m] = 0.0; }
+  bool have = false, exhausted = false;
+  int st_next = 0, st_avail = 0;
+  for (;;) {
+    __syncwarp();
+    const unsigned need = __ballot_sync(0xffffffffu, !have);
+    if (need) {
+      if (st_next == st_avail && !exhausted) {
+        int base = 0;
+        if (lane == 0) base = atomicAdd(work_counter, 32);
+        base = __shfl_sync(0xffffffffu, base, 0);
+        const int cnt = min(32, n - base);
+        if (cnt <= 0) {
+          exhausted = true;
+        } else {
+          const uint4* src = reinterpret_cast<const uint4*>(esc.buf + base);
+          for (int i = lane; i < cnt * PH_U4; i += 32) stage[i] = __ldg(src + i);
+          st_next = 0; st_avail = cnt;
+        }
+        __syncwarp();
+      }
+      const int left = st_avail - st_next;
+      if (left > 0) {
+        const int rank = __popc(need & lt_mask);
+        if (!have && rank < left) {
+          lane_load(L, reinterpret_cast<const Photon*>(stage) + st_next + rank);
+          have = true;
+        }
+        st_next += min(__popc(need), left);
+        __syncwarp();
+      } else if (exhausted && need == 0xffffffffu) {
         break;
       }
-      if (L.w < P.w_min) {
-        double ux, ur;
-        uniform_pair(P, TAG_STEP, L.id0, L.id1, L.id2, L.nstep, ux, ur);
-        const Lane T = L;
-        L.w = roulette(P, T, ur, stats, trace);
-        if (L.w < 0.0) break;
-      }
-      const double dl = step_size(P, L.x, L.k);
-      double x1[4], k1[4], a1[4];
-      Geom G;
-      bool capped;
-      c_viters += push<KERR>(P, L.x, L.k, L.a, dl, x1, k1, a1, G, capped);
-      c_capped += capped ? 1 : 0;
-#pragma unroll
-      for (int m = 0; m < 4; m++) { L.x[m] = x1[m]; L.k[m] = k1[m]; L.a[m] = a1[m]; }
-      L.nstep++; c_steps++;
     }
+    if (!have) continue;
+    if (stop_tests<KERR>(P, L, tally, stats, trace)) { have = false; continue; }
+    if (L.x[1] < P.x1hi) {                                 // back inside the grid
+      L.nua_a = 0.0; L.nua_s = 0.0; L.bias = 1.0;          // opacities at a vacuum point
+      const int slot = atomicAdd(ret.count, 1);
+      if (slot < ret.capacity) lane_store(L, ret.buf + slot);
+      atomicAdd(&stats->n[SN_REENTER], 1ull);
+      have = false; continue;
+    }
+    if (L.w < P.w_min) {
+      double ux, ur;
+      uniform_pair(P, TAG_STEP, L.id0, L.id1, L.id2, L.nstep, ux, ur);
+      const Lane T = L;
+      L.w = roulette(P, T, ur, stats, trace);
+      if (L.w < 0.0) { have = false; continue; }
+    }
+    const double dl = step_size(P, L.x, L.k);
+    double x1[4], k1[4], a1[4];
+    Geom G;
+    bool capped;
+    c_viters += push<KERR>(P, L.x, L.k, L.a, dl, x1, k1, a1, G, capped);
+    c_capped += capped ? 1 : 0;
+#pragma unroll
+    for (int m = 0; m < 4; m++) { L.x[m] = x1[m]; L.k[m] = k1[m]; L.a[m] = a1[m]; }
+    L.nstep++; c_steps++;
   }
   for (int o = 16; o > 0; o >>= 1) {
     c_steps += __shfl_xor_sync(0xffffffffu, c_steps, o);
@@ -886,11 +927,13 @@ cudaError_t launch_track(const DevParams& P, int phase, const Photon* in, const 
   return cudaGetLastError();
 }
 
-cudaError_t launch_escape(const DevParams& P, Queue esc, Queue ret, Tally tally, DevStats* stats, TraceBuf trace,
-                          int n_sm, cudaStream_t st) {
+cudaError_t launch_escape(const DevParams& P, Queue esc, int* work_counter, Queue ret, Tally tally, DevStats* stats,
+                          TraceBuf trace, int n_sm, cudaStream_t st) {
   const int grid = n_sm * GM_ESC_MINBLOCKS;
-  if (P.metric_kind == 1) escape_kernel<true><<<grid, 128, 0, st>>>(P, esc, ret, tally, stats, trace);
-  else escape_kernel<false><<<grid, 128, 0, st>>>(P, esc, ret, tally, stats, trace);
+  cudaError_t e = cudaMemsetAsync(work_counter, 0, sizeof(int), st);
+  if (e != cudaSuccess) return e;
+  if (P.metric_kind == 1) escape_kernel<true><<<grid, 128, 0, st>>>(P, esc, work_counter, ret, tally, stats, trace);
+  else escape_kernel<false><<<grid, 128, 0, st>>>(P, esc, work_counter, ret, tally, stats, trace);
   return cudaGetLastError();
 }
 
