@@ -172,7 +172,11 @@ constexpr int PH_U4 = sizeof(Photon) / 16;          // 10 x 16 B per record
 // The 2-D gather (4 zone records) is staged through shared memory with asynchronous copies; the 3-D one (8 records,
 // 16 KB of slots per warp) is not: its slots would leave no L1 for the line sharing between neighbouring records,
 // and measured slower either way (profiles/r01e).  Refill stage: 32 records (5 KB) per warp.
+#ifdef GM_NO_STAGED
+__host__ __device__ constexpr bool track_staged_gather(bool) { return false; }
+#else
 __host__ __device__ constexpr bool track_staged_gather(bool threed) { return !threed; }
+#endif
 __host__ __device__ constexpr int track_stage_records(bool) { return 32; }
 __host__ __device__ constexpr int track_smem_bytes(bool threed) {
   return TRACK_WARPS * (track_stage_records(threed) * PH_U4 + (track_staged_gather(threed) ? 4 * 4 * 32 : 0)) * 16;
