@@ -385,6 +385,8 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
   bool exhausted = false;               // warp-uniform
   unsigned long long c_steps = 0, c_viters = 0;
   double c_absorbed = 0.0;
+  unsigned c_rk = 0;                    // roulette kills of this thread and their weight
+  double c_rkw = 0.0;
 
   for (;;) {
     __syncwarp();
@@ -432,9 +434,18 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
       double ur;
       uniform_pair(P, TAG_STEP, L.id0, L.id1, L.id2, L.nstep, ux, ur);
       if (L.w < P.w_min && !(L.flags & FLAG_ROULETTED)) {
+#ifdef GM_ROUL_CALL
         const Lane T = L;
         L.w = roulette(P, T, ur, stats, trace);
         if (L.w < 0.0) { have = false; continue; }
+#else
+        // most roulettes kill (survival 1/roulette): counted in registers, no call and no lane copy unless a
+        // trace buffer wants the record
+        if (ur >= P.inv_roulette && !trace.rec) { c_rk++; c_rkw += L.w; have = false; continue; }
+        const Lane T = L;
+        L.w = roulette(P, T, ur, stats, trace);
+        if (L.w < 0.0) { have = false; continue; }
+#endif
         L.flags |= FLAG_ROULETTED;                        // cleared when the step is committed
       }
       dl = step_size(P, L.x, L.k);
@@ -564,10 +575,14 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
     c_viters += __shfl_xor_sync(0xffffffffu, c_viters, o);
   }
   c_absorbed = warp_sum(c_absorbed);
+  c_rkw = warp_sum(c_rkw);
+  c_rk = __reduce_add_sync(0xffffffffu, c_rk);
   if (lane == 0) {
     stat_add_n(stats, SN_STEPS, c_steps);
     stat_add_n(stats, SN_VITERS, c_viters);
     stat_add_s(stats, SS_ABSORBED, c_absorbed);
+    stat_add_n(stats, SN_ROUL_KILLED, c_rk);
+    stat_add_s(stats, SS_ROUL_KILLED, c_rkw);
   }
 }
 
