@@ -37,10 +37,10 @@ METRIC = "superphotons/s tracked (incl. scattering)"
 UNIT = "superphotons/s"
 # algorithmic FP64 flop per geodesic step (dadd + dmul + 2 dfma predicated-on thread
 # instructions of the kernel divided by the steps it committed, counted with ncu on each workload class with the
-# single mixed tracker pass, so that no redone step is counted -- profiles/r01d_flop_per_step.md -- and then
+# single mixed tracker pass, so that no redone step is counted -- profiles/r01f_final.md -- and then
 # frozen).  "track": in-grid step of track_kernel; "escape": free-flight step of escape_kernel.
-FLOP_PER_STEP = {"flat": {"track": 676.3, "escape": 207.9}, "kerr": {"track": 693.2, "escape": 367.1},
-                 "kerr3d": {"track": 795.1, "escape": 367.1}}
+FLOP_PER_STEP = {"flat": {"track": 717.6, "escape": 208.0}, "kerr": {"track": 704.7, "escape": 368.2},
+                 "kerr3d": {"track": 807.5, "escape": 368.2}}
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant launch (cold tracker pass over 1.09e6 primaries,
 # cfg2 at Ns=3e6) from the ncu --set full capture of profiles/r01c_phase_passes.md; quoted for cfg2 only
 TRAFFIC_BYTES_PER_LAUNCH = {2: 86.9e6 + 78.5e6}

@@ -383,7 +383,7 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
   int ev_it = 0;                        // PHASE_COLD: Verlet iterations counted for the attempt that found the event
   int st_next = 0, st_avail = 0;        // staged records [st_next, st_avail); warp-uniform
   bool exhausted = false;               // warp-uniform
-  unsigned long long c_steps = 0, c_viters = 0;
+  unsigned c_steps = 0, c_viters = 0;            // per thread and launch: far below 2^32
   double c_absorbed = 0.0;
   unsigned c_rk = 0;                    // roulette kills of this thread and their weight
   double c_rkw = 0.0;
@@ -481,7 +481,7 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
           const int slot = atomicAdd(park.count, 1);
           if (slot < park.capacity) lane_store(L, park.buf + slot);
           if (mode != 0) {                                 // the attempt of this step is redone: uncount it
-            c_viters -= (unsigned long long)abs(ev_it);
+            c_viters -= (unsigned)abs(ev_it);
             if (ev_it < 0) atomicAdd(&stats->n[SN_VCAPPED], ~0ull);
           }
           have = false; mode = 0;
@@ -570,16 +570,18 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
     }
   }
   // flush thread-local counters
+  // (c_viters may have wrapped below zero in a thread that uncounted a redone attempt: read as a signed number)
+  long long w_steps = c_steps, w_viters = (int)c_viters;
   for (int o = 16; o > 0; o >>= 1) {
-    c_steps += __shfl_xor_sync(0xffffffffu, c_steps, o);
-    c_viters += __shfl_xor_sync(0xffffffffu, c_viters, o);
+    w_steps += __shfl_xor_sync(0xffffffffu, w_steps, o);
+    w_viters += __shfl_xor_sync(0xffffffffu, w_viters, o);
   }
   c_absorbed = warp_sum(c_absorbed);
   c_rkw = warp_sum(c_rkw);
   c_rk = __reduce_add_sync(0xffffffffu, c_rk);
   if (lane == 0) {
-    stat_add_n(stats, SN_STEPS, c_steps);
-    stat_add_n(stats, SN_VITERS, c_viters);
+    stat_add_n(stats, SN_STEPS, (unsigned long long)w_steps);
+    stat_add_n(stats, SN_VITERS, (unsigned long long)w_viters);
     stat_add_s(stats, SS_ABSORBED, c_absorbed);
     stat_add_n(stats, SN_ROUL_KILLED, c_rk);
     stat_add_s(stats, SS_ROUL_KILLED, c_rkw);
@@ -606,7 +608,7 @@ escape_kernel(const __grid_constant__ DevParams P, Queue esc, int* work_counter,
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const unsigned lt_mask = (1u << lane) - 1u;
   uint4* stage = s_stage[wid];
-  unsigned long long c_steps = 0, c_viters = 0, c_capped = 0;
+  unsigned c_steps = 0, c_viters = 0;             // per thread and launch: far below 2^32
   Lane L;
   L.w = 0.0; L.nua_a = 0.0; L.nua_s = 0.0; L.bias = 1.0;
   L.id0 = L.id1 = L.id2 = L.nstep = L.jscat = 0u; L.nsc = 0; L.root = -1; L.flags = 0;
@@ -677,21 +679,20 @@ escape_kernel(const __grid_constant__ DevParams P, Queue esc, int* work_counter,
     Geom G;
     bool capped;
     c_viters += push<KERR>(P, L.x, L.k, L.a, dl, x1, k1, a1, G, capped);
-    c_capped += capped ? 1 : 0;
+    if (capped) atomicAdd(&stats->n[SN_VCAPPED], 1ull);
 #pragma unroll
     for (int m = 0; m < 4; m++) { L.x[m] = x1[m]; L.k[m] = k1[m]; L.a[m] = a1[m]; }
     L.nstep++; c_steps++;
   }
+  unsigned long long w_steps = c_steps, w_viters = c_viters;
   for (int o = 16; o > 0; o >>= 1) {
-    c_steps += __shfl_xor_sync(0xffffffffu, c_steps, o);
-    c_viters += __shfl_xor_sync(0xffffffffu, c_viters, o);
-    c_capped += __shfl_xor_sync(0xffffffffu, c_capped, o);
+    w_steps += __shfl_xor_sync(0xffffffffu, w_steps, o);
+    w_viters += __shfl_xor_sync(0xffffffffu, w_viters, o);
   }
   if ((threadIdx.x & 31) == 0) {
-    stat_add_n(stats, SN_STEPS, c_steps);
-    stat_add_n(stats, SN_STEPS_FREE, c_steps);
-    stat_add_n(stats, SN_VITERS, c_viters);
-    stat_add_n(stats, SN_VCAPPED, c_capped);
+    stat_add_n(stats, SN_STEPS, w_steps);
+    stat_add_n(stats, SN_STEPS_FREE, w_steps);
+    stat_add_n(stats, SN_VITERS, w_viters);
   }
 }
 
