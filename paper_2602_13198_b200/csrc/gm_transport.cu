@@ -538,7 +538,7 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
         const double b = 0.5 * (L.bias + b1);
         // w/b >= w_min is the other condition of the event (G21): a weight below half of w_min b cannot meet it,
         // whatever the rounding of the division, and needs no logarithm
-        if (bt > ux && L.w > 0.5 * P.w_min * b) {
+        if (bt > ux && L.w >= 0.5 * P.w_min * b) {        // >=: with w_min = 0 a weight of exactly 0 still scatters
           const double xr = -log(1.0 - ux);
           if (bt > xr && L.w / b >= P.w_min) {
             mode = 1; ev_f = xr / bt; ev_b = b; ev_tau = tau_a;

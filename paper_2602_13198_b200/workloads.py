@@ -74,15 +74,21 @@ def dtheta_dx2(x2, hslope):
 # cfg 0 / 1 : uniform synchrotron sphere in flat space
 # --------------------------------------------------------------------------
 def sphere(n_e=1e13, thetae=10.0, B_gauss=1.0, R=1e3, n1=32, n2=16,
-           Ns=1e5, seed=1, scattering=False, **over):
+           Ns=1e5, seed=1, scattering=False, r_out=None, partial_sub=0, **over):
     """Uniform sphere, radius R cm, static fluid, field along z (PAPER.md:221-229,
-    with the G5 correction of Eq. 31 for x1 = ln r)."""
+    with the G5 correction of Eq. 31 for x1 = ln r).
+
+    r_out (default R): outer edge of the grid.  With r_out > R the sphere surface falls inside a radial zone, as
+    it does on the paper's grid.  partial_sub = 0: abrupt cutoff (a zone holds gas if its
+    centre lies inside R); partial_sub = m: the paper's partial-cell treatment -- each zone is divided into an
+    m x m sub-grid and its density is scaled by the fraction of sub-cell centres inside R (m = 5 in the paper)."""
     p = default_params()
     L_unit = 1.0
     M_unit = (MP + ME) * L_unit ** 3          # => Ne_unit = 1, rho == n_e
     B_unit = CL * math.sqrt(4.0 * math.pi * M_unit / L_unit ** 3)
     x1_0 = math.log(R * math.exp(-3.0))
-    dx1 = 3.0 / n1
+    x1_end = math.log(R if r_out is None else r_out)
+    dx1 = 3.0 / n1 if r_out is None else (x1_end - x1_0) / n1
     dx2 = 1.0 / n2
     p.update(seed=seed, Ns_target=float(Ns), metric_kind=0, a_spin=0.0, hslope=1.0,
              startx=[0.0, x1_0, 0.0, 0.0], dx=[1.0, dx1, dx2, 2.0 * math.pi],
@@ -99,7 +105,13 @@ def sphere(n_e=1e13, thetae=10.0, B_gauss=1.0, R=1e3, n1=32, n2=16,
     B0 = B_gauss / B_unit
     prim = np.zeros((n1, n2, 1, NPRIM))
     prim[..., 0] = n_e
-    prim[..., 1] = 1e-3 * n_e                  # unused in thetae_mode 0
+    if r_out is not None:
+        m = max(1, int(partial_sub))
+        # fraction of the m x m sub-cell centres (in x1, x2) of each zone that lie inside R; r depends on x1 only
+        sub = x1_0 + (np.arange(n1)[:, None] + (np.arange(m)[None, :] + 0.5) / m) * dx1
+        frac = (np.exp(sub) < R).mean(axis=1)
+        prim[..., 0] = n_e * frac[:, None, None]
+    prim[..., 1] = 1e-3 * prim[..., 0]         # unused in thetae_mode 0
     prim[:, :, 0, 5] = B0 * np.cos(th) / r
     prim[:, :, 0, 6] = -B0 * np.sin(th) / (r * dth)
     p.update(over)

@@ -340,6 +340,29 @@ def test_config4_analog_scattering_small(gm):
     _compare_traces(o, g, ids, fork_budget=5e-3)
 
 
+@pytest.mark.parametrize("scattering", [False, True])
+def test_partial_cell_sphere_boundary(gm, scattering):
+    """the sphere surface cuts a radial zone; densities scaled by the 5 x 5
+    sub-grid fraction, empty zones beyond.  Counts bit-exact, traces and spectrum against the oracle."""
+    import math
+    n1 = 96
+    dx1 = 3.0 / (n1 - 1.65)
+    kw = dict(r_out=1e3 * math.exp(1.65 * dx1), partial_sub=5)
+    if scattering:
+        p, prim = wl.sphere(1.503e19, 4.0, 1.0, 1e3, n1, 16, 1e5, 5, True, bias0=25.0, bias_p_theta=0, bias_q_nsc=2, **kw)
+    else:
+        p, prim = wl.sphere(1e13, 10.0, 1.0, 1e3, n1, 16, 1e5, 5, False, **kw)
+    assert 0 < prim[n1 - 2, 0, 0, 0] < prim[0, 0, 0, 0] and prim[n1 - 1, 0, 0, 0] == 0.0
+    o, g = _pair(gm, p, prim)
+    assert np.array_equal(o.zone_counts(), g.zone_counts())
+    assert g.zone_counts().reshape(n1, 16)[n1 - 1].sum() == 0 and g.zone_counts().reshape(n1, 16)[n1 - 2].sum() > 0
+    o.run(); g.run()
+    _compare_stats(o, g, rel=1e-6)
+    _compare_spectra(o, g, min_count=300)
+    ids = np.arange(0, g.n_primaries, 17)
+    _compare_traces(o, g, ids, fork_budget=2e-3)
+
+
 @pytest.mark.parametrize("cfg,pairs,k_cold", [(2, 1, 1), (2, 2, 4), (2, 3, 2), (3, 2, 3), (4, 2, 1)])
 def test_hot_cold_phase_passes_change_no_history(gm, cfg, pairs, k_cold):
     """Tracker schedule (gm_set_phase_passes): a history is a pure function of its record, so
