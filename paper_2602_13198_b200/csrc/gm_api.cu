@@ -30,6 +30,7 @@ struct gm_ctx {
   Photon *d_parkA = nullptr, *d_parkB = nullptr;   // hot/cold pass hand-over queues (esc_records each)
   int phase_pairs = -1, k_cold = 4;                // -1: automatic (decided by a pilot batch, see gm_run)
   int auto_pairs = -1;                             // the pilot's decision (-1: not taken yet)
+  int carry_lanes = 4;                             // straggler hand-over threshold (0: off); GPUMONTY_B200_CARRY overrides
   double pilot_cold_fraction = -1.0;
   long long esc_records = 0;
   long long batch_primaries = 0, queue_records = 0;   // allocated sizes
@@ -230,6 +231,7 @@ int gm_create(gm_ctx** out, const gm_params* p) {
   ctx->tally_snap.Q = ctx->tally_snap.A + nb; ctx->tally_snap.W = ctx->tally_snap.A + 2 * nb;
   ctx->tally_snap.n = (unsigned long long*)(ctx->tally_snap.A + 3 * nb);
   fill_dev_params(ctx);
+  if (const char* e = getenv("GPUMONTY_B200_CARRY")) ctx->carry_lanes = atoi(e) < 0 ? 0 : (atoi(e) > 32 ? 32 : atoi(e));
   // parameter-free tables (S0)
   cudaError_t te = gm_build_tables(ctx, nullptr) == GM_OK ? cudaSuccess : cudaErrorUnknown;
   if (te == cudaSuccess) te = cudaMemset(ctx->tally.A, 0, (size_t)nb * 4 * sizeof(double));
@@ -425,19 +427,24 @@ static int run_batch(gm_ctx* ctx, long long first, int n, const long long* d_ids
   int mq = 0, round = 0;
   for (;;) {
     // generations 0..layers without a host round trip; afterwards only while re-entrants keep a queue non-empty
-    const int last = round + layers;
+    // first block: the nominal generations; afterwards one round per host check (re-entrants from free flight and
+    // the descendants of stragglers that were carried into the last nominal round)
+    const bool first_block = round == 0;
+    const int last = first_block ? layers : round;
     for (; round <= last && round < MAXROUND; round++) {
       Queue out{(round & 1) ? ctx->d_qB : ctx->d_qA, cnt + 3 + round, qcap};
+      // stragglers of every generation but the last nominal one continue in the next generation's launch
+      const int carry = (ctx->carry_lanes > 0 && first_block && round < last) ? ctx->carry_lanes : 0;
       CK(cudaMemsetAsync(esc.count, 0, sizeof(int), st));
       if (pairs == 0) {
-        TIMED(GM_T_TRACK, st, launch_track(ctx->P, 0, in, in_count, in_cap, cnt + 1, out, esc, nopark, 0, tally, stats, trace, ctx->n_sm, st));
+        TIMED(GM_T_TRACK, st, launch_track(ctx->P, 0, in, in_count, in_cap, cnt + 1, out, esc, nopark, 0, carry, tally, stats, trace, ctx->n_sm, st));
       } else {
         // hot pass (in -> parkA), cold pass (parkA -> parkB), hot pass (parkB -> parkA), ... ; the last cold
         // pass handles hot plasma in place.  Every queue is fully consumed before it is refilled.
         const Photon* pin = in; const int* pcount = in_count; int pcap = in_cap;
         for (int pp = 0; pp < pairs; pp++) {
           CK(cudaMemsetAsync(parkA.count, 0, sizeof(int), st));
-          TIMED(GM_T_TRACK, st, launch_track(ctx->P, 1, pin, pcount, pcap, cnt + 1, out, esc, parkA, ctx->k_cold, tally, stats, trace, ctx->n_sm, st));
+          TIMED(GM_T_TRACK, st, launch_track(ctx->P, 1, pin, pcount, pcap, cnt + 1, out, esc, parkA, ctx->k_cold, carry, tally, stats, trace, ctx->n_sm, st));
           if (deciding) {
             int parked = 0;
             CK(cudaMemcpyAsync(&parked, parkA.count, sizeof(int), cudaMemcpyDeviceToHost, st));
@@ -451,10 +458,10 @@ static int run_batch(gm_ctx* ctx, long long first, int n, const long long* d_ids
             if (ctx->auto_pairs == 0) pairs = 1;           // finish this generation with the mixed pass, then none
           }
           if (pp >= pairs - 1) {
-            TIMED(GM_T_TRACK, st, launch_track(ctx->P, 0, parkA.buf, parkA.count, parkA.capacity, cnt + 1, out, esc, nopark, 0, tally, stats, trace, ctx->n_sm, st));
+            TIMED(GM_T_TRACK, st, launch_track(ctx->P, 0, parkA.buf, parkA.count, parkA.capacity, cnt + 1, out, esc, nopark, 0, carry, tally, stats, trace, ctx->n_sm, st));
           } else {
             CK(cudaMemsetAsync(parkB.count, 0, sizeof(int), st));
-            TIMED(GM_T_TRACK, st, launch_track(ctx->P, 2, parkA.buf, parkA.count, parkA.capacity, cnt + 1, out, esc, parkB, 0, tally, stats, trace, ctx->n_sm, st));
+            TIMED(GM_T_TRACK, st, launch_track(ctx->P, 2, parkA.buf, parkA.count, parkA.capacity, cnt + 1, out, esc, parkB, 0, carry, tally, stats, trace, ctx->n_sm, st));
             pin = parkB.buf; pcount = parkB.count; pcap = parkB.capacity;
           }
         }

@@ -43,9 +43,11 @@ cudaError_t launch_emit(const DevParams& P, const ZoneArrays& Z, long nz, long l
 // events append proto-children (parent state at the event) to `out`, leavers go to `esc` (the caller resets
 // esc.count once per generation).  phase 0: everything in place; 1 (hot pass): a lane that was cold for k_cold
 // committed steps is moved to `park`; 2 (cold pass): a lane that meets hot plasma is moved to `park`.
+// carry_lanes > 0: a warp whose input is exhausted hands its last <= carry_lanes flying superphotons to `esc`
+// marked as stragglers; launch_escape passes them on to `ret` (the next generation's input).
 cudaError_t launch_track(const DevParams& P, int phase, const Photon* in, const int* in_count, int in_capacity,
-                         int* work_counter, Queue out, Queue esc, Queue park, int k_cold, Tally tally, DevStats* stats,
-                         TraceBuf trace, int n_sm, cudaStream_t st);
+                         int* work_counter, Queue out, Queue esc, Queue park, int k_cold, int carry_lanes, Tally tally,
+                         DevStats* stats, TraceBuf trace, int n_sm, cudaStream_t st);
 // free flight of the leavers to r_max (record) ; a superphoton that re-enters the grid is appended to `ret`
 cudaError_t launch_escape(const DevParams& P, Queue esc, int* work_counter, Queue ret, Tally tally, DevStats* stats,
                           TraceBuf trace, int n_sm, cudaStream_t st);

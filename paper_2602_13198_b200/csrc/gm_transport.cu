@@ -16,7 +16,8 @@
 namespace gm {
 
 constexpr int FLAG_ROOT = 1, FLAG_DEAD = 2;
-constexpr int FLAG_ROULETTED = 4;   // the roulette of step `nstep` was already played (record moved between passes)
+constexpr int FLAG_ROULETTED = 4;
+constexpr int FLAG_CARRY = 8;       // straggler handed to the next generation's launch through the free-flight queue   // the roulette of step `nstep` was already played (record moved between passes)
 
 // ---- block-level stats helper ---------------------------------------------------------------------
 __device__ __forceinline__ void stat_add_n(DevStats* st, int which, unsigned long long v) {
@@ -359,8 +360,8 @@ __global__ void __maxnreg__(GM_TRACK_MAXNREG)
 __global__ void __launch_bounds__(TRACK_THREADS, PHASE == 2 ? GM_COLD_MINBLOCKS : GM_TRACK_MINBLOCKS)
 #endif
 track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in, const int* __restrict__ in_count, int in_capacity,
-             int* work_counter, Queue out, Queue esc, Queue park, int k_cold, Tally tally, DevStats* stats,
-             TraceBuf trace) {
+             int* work_counter, Queue out, Queue esc, Queue park, int k_cold, int carry_lanes, Tally tally,
+             DevStats* stats, TraceBuf trace) {
   // dynamic shared memory: per warp the next STAGE_REC records (refill stage) and the gather slots of its lanes
   extern __shared__ uint4 s_dyn[];
   constexpr int STAGE_REC = track_stage_records(THREED);
@@ -392,6 +393,21 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
     __syncwarp();
     // ---- refill the stopped lanes of this warp together ----
     const unsigned need = __ballot_sync(0xffffffffu, !have);
+    // Stragglers: once this warp's input is exhausted and only `carry_lanes` or fewer of its lanes still fly, their
+    // records go to the free-flight queue marked FLAG_CARRY; escape_kernel hands them unchanged to the next
+    // generation's launch, where they continue inside full warps.  The launch then ends with its bulk instead of
+    // its longest history (a superphoton grazing the polar axis takes thousands of steps).  Only lanes at a step
+    // boundary (mode 0) are handed over, so nothing is counted twice.
+    if (carry_lanes > 0 && exhausted && st_next == st_avail && need != 0xffffffffu &&
+        __popc(~need) <= carry_lanes && __ballot_sync(0xffffffffu, have && mode != 0) == 0u) {
+      if (have) {
+        L.flags |= FLAG_CARRY;
+        const int slot = atomicAdd(esc.count, 1);
+        if (slot < esc.capacity) lane_store(L, esc.buf + slot);
+        have = false;
+      }
+      break;
+    }
     if (need) {
       if (st_next == st_avail && !exhausted) {
         int base = 0;
@@ -656,6 +672,12 @@ escape_kernel(const __grid_constant__ DevParams P, Queue esc, int* work_counter,
       }
     }
     if (!have) continue;
+    if (L.flags & FLAG_CARRY) {                            // a tracker straggler: on to the next generation, as it is
+      L.flags &= ~FLAG_CARRY;
+      const int slot = atomicAdd(ret.count, 1);
+      if (slot < ret.capacity) lane_store(L, ret.buf + slot);
+      have = false; continue;
+    }
     if (L.x[2] < 0.0) { L.x[2] = -L.x[2]; L.k[2] = -L.k[2]; L.a[2] = -L.a[2]; L.x[3] += C_PI; }
     if (L.x[2] > 1.0) { L.x[2] = 2.0 - L.x[2]; L.k[2] = -L.k[2]; L.a[2] = -L.a[2]; L.x[3] += C_PI; }
     if (L.x[1] >= P.lnr_max) { arrived = true; have = false; continue; }       // recorded at the next refill
@@ -971,13 +993,13 @@ cudaError_t launch_emit(const DevParams& P, const ZoneArrays& Z, long nz, long l
 }
 
 cudaError_t launch_track(const DevParams& P, int phase, const Photon* in, const int* in_count, int in_capacity,
-                         int* work_counter, Queue out, Queue esc, Queue park, int k_cold, Tally tally, DevStats* stats,
-                         TraceBuf trace, int n_sm, cudaStream_t st) {
+                         int* work_counter, Queue out, Queue esc, Queue park, int k_cold, int carry_lanes, Tally tally,
+                         DevStats* stats, TraceBuf trace, int n_sm, cudaStream_t st) {
   cudaError_t e = cudaMemsetAsync(work_counter, 0, sizeof(int), st);
   if (e != cudaSuccess) return e;
   const int grid = n_sm * (phase == PHASE_COLD ? GM_COLD_MINBLOCKS : GM_TRACK_MINBLOCKS);
   const bool kerr = P.metric_kind == 1, td = P.n3 > 1;
-#define GM_TRACK_ARGS P, in, in_count, in_capacity, work_counter, out, esc, park, k_cold, tally, stats, trace
+#define GM_TRACK_ARGS P, in, in_count, in_capacity, work_counter, out, esc, park, k_cold, carry_lanes, tally, stats, trace
   const int smem = track_smem_bytes(td);
   static bool attr_set = false;
   if (!attr_set) {                       // > 48 KB of dynamic shared memory needs the opt-in, once per kernel

@@ -340,6 +340,34 @@ def test_config4_analog_scattering_small(gm):
     _compare_traces(o, g, ids, fork_budget=5e-3)
 
 
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_straggler_carry_over_changes_no_history(gm, cfg, monkeypatch):
+    """A warp whose input is exhausted hands its last few flying superphotons to the next generation's launch
+    (threshold read from GPUMONTY_B200_CARRY at gm_create).  Off, default and the extreme
+    setting (every warp hands over all 32 lanes as soon as its input ends) must give identical histories."""
+    p, prim = (wl.config1(Ns=5e4) if cfg == 1 else wl.config2(Ns=2e4))
+    res = []
+    for carry in ("0", "4", "32"):
+        monkeypatch.setenv("GPUMONTY_B200_CARRY", carry)
+        g = gm.GPUMonty(p)
+        g.set_grid(prim)
+        g.prepare()
+        g.run()
+        ids = np.arange(0, g.n_primaries, 7)
+        res.append((g.stats(), g.tally(), g.trace(ids)))
+    s0, (A0, Q0, W0, n0), t0 = res[0]
+    for s1, (A1, Q1, W1, n1), t1 in res[1:]:
+        for k in s0:
+            if k.startswith("n_"):
+                assert s0[k] == s1[k], (k, s0[k], s1[k])
+            else:
+                assert s1[k] == pytest.approx(s0[k], rel=1e-11, abs=1e-300), k
+        assert np.array_equal(n0, n1) and np.allclose(A0, A1, rtol=1e-11, atol=0)
+        for f in ("fate", "nstep", "inu", "ith", "jscat", "fam_nspawn"):
+            assert np.array_equal(t0[f], t1[f]), f
+        assert np.array_equal(t0["w"], t1["w"]) and np.array_equal(t0["x"], t1["x"])
+
+
 @pytest.mark.parametrize("scattering", [False, True])
 def test_partial_cell_sphere_boundary(gm, scattering):
     """the sphere surface cuts a radial zone; densities scaled by the 5 x 5
