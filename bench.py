@@ -42,8 +42,8 @@ UNIT = "superphotons/s"
 FLOP_PER_STEP = {"flat": {"track": 717.6, "escape": 208.0}, "kerr": {"track": 704.7, "escape": 368.2},
                  "kerr3d": {"track": 807.5, "escape": 368.2}}
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant launch (cold tracker pass over 1.09e6 primaries,
-# cfg2 at Ns=3e6) from the ncu --set full capture of profiles/r01c_phase_passes.md; quoted for cfg2 only
-TRAFFIC_BYTES_PER_LAUNCH = {2: 86.9e6 + 78.5e6}
+# cfg2 at Ns=3e6) from the ncu --set full capture of profiles/r01g_carry_over.md; quoted for cfg2 only
+TRAFFIC_BYTES_PER_LAUNCH = {2: 85.4e6 + 76.2e6}
 WORKLOAD_NAMES = {0: "cfg0 thin synchrotron sphere 32x16, Ns=1e5", 1: "cfg1 scattering sphere 32x16, Ns=1e6",
                   2: "cfg2 Kerr FM torus 256x256, Ns=1e7", 3: "cfg3 3-D perturbed torus 192x128x128, Ns=1e7",
                   4: "cfg4 Kerr torus x1e3 density (analog scattering), Ns=1e6"}
