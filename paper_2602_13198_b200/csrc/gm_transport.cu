@@ -839,7 +839,13 @@ __device__ inline bool compton_event(const DevParams& P, const Geom& G, const Pl
 }
 
 template <bool KERR, bool THREED>
-__global__ void __launch_bounds__(128) compton_kernel(const DevParams P, Queue q, DevStats* stats, TraceBuf trace) {
+// The event body is a chain of rejection loops (Maxwell-Juttner, Klein-Nishina): divergent and latency-bound, so
+// it wants warps, not registers.  Measured per cfg2 step: 254 registers (8 warps/SM) 17.8 ms, 128 (16) 13.2,
+// 96 (20) 11.0, 80 (24) 10.3, 64 (32) 9.7 -- the spills are cheaper than the idle issue slots.
+#ifndef GM_COMPTON_MINBLOCKS
+#define GM_COMPTON_MINBLOCKS 8
+#endif
+__global__ void __launch_bounds__(128, GM_COMPTON_MINBLOCKS) compton_kernel(const DevParams P, Queue q, DevStats* stats, TraceBuf trace) {
   const int n = min(*q.count, q.capacity);
   unsigned long long c_spawn = 0, c_bad = 0;
   double s_bad = 0.0;
@@ -1039,7 +1045,7 @@ cudaError_t launch_escape(const DevParams& P, Queue esc, int* work_counter, Queu
 }
 
 cudaError_t launch_compton(const DevParams& P, Queue q, DevStats* stats, TraceBuf trace, int n_sm, cudaStream_t st) {
-  const int grid = n_sm * 4;
+  const int grid = n_sm * (GM_COMPTON_MINBLOCKS > 4 ? GM_COMPTON_MINBLOCKS : 4);
   GM_DISPATCH(compton_kernel, grid, 128, st, P, q, stats, trace);
   return cudaGetLastError();
 }
