@@ -54,7 +54,10 @@ __device__ __forceinline__ void tally_add(const Tally& T, int bin, double wE, do
 // tetrad with axis 1 along b (G13)
 // =====================================================================================================
 template <bool KERR>
-__global__ void __launch_bounds__(128) emit_kernel(const DevParams P, ZoneArrays Z, long nz, long long first,
+#ifndef GM_EMIT_MINBLOCKS
+#define GM_EMIT_MINBLOCKS 6
+#endif
+__global__ void __launch_bounds__(128, GM_EMIT_MINBLOCKS) emit_kernel(const DevParams P, ZoneArrays Z, long nz, long long first,
                                                    int n, const long long* __restrict__ ids, Photon* __restrict__ out,
                                                    int* out_count, DevStats* stats, gm_emit_rec* __restrict__ erec,
                                                    int with_root) {
