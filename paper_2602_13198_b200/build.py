@@ -43,7 +43,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         if r.returncode != 0:
             raise RuntimeError("nvcc failed: " + " ".join(cmd))
         with open(cmd[-1].replace(".o", ".ptxas.txt"), "w") as f:     # registers / spills per kernel
-            f.write(r.stderr)
+            # (compile times dropped: the listing then changes only when the code does)
+            f.write("".join(l for l in r.stderr.splitlines(True) if "Compile time" not in l))
 
     if jobs:
         with ThreadPoolExecutor(max_workers=len(jobs)) as ex:
