@@ -205,6 +205,19 @@ void orc_plasma_at(void* h, const double* x, double* out) {
   for (int m = 0; m < 4; m++) { out[3 + m] = S.ucon[m]; out[7 + m] = S.bcon[m]; }
   out[11] = S.vacuum ? 1.0 : 0.0;
 }
+// fluid-frame photon energy and field angle at x for wavevector k: out = eps, cos(theta_B), nu*alpha_abs,
+// nu*alpha_scat, bias (n_sc = nsc), vacuum flag  (6 doubles)
+void orc_fluid_frame(void* h, const double* x, const double* k, int nsc, double* out) {
+  Context* C = (Context*)h;
+  if (C->T.lnK2.empty() || (C->P.scattering_on && !C->T.have_sigh)) { ensure_tables(C->P.scattering_on != 0); C->T = g_tables; }
+  Geom G; geom_func(C->P, x, &G);
+  Plasma S; plasma_at(C->P, C->un, C->prim.data(), x, G, &S);
+  for (int i = 0; i < 6; i++) out[i] = 0.0;
+  out[5] = S.vacuum ? 1.0 : 0.0;
+  if (S.vacuum) return;
+  fluid_frame(*C, k, G, S, &out[0], &out[1]);
+  opacities(*C, x, k, G, S, &out[2], &out[3], &out[4], nsc);
+}
 void orc_sample_mj(double thetae, uint64_t seed, int n, double* gamma_out) {
   for (int i = 0; i < n; i++) {
     Stream rs(seed, TAG_SCAT, (uint32_t)i, 0u, 0u);

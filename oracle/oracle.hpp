@@ -130,7 +130,8 @@ struct Stats {
       n_maxstep, n_outofrange, n_steps_total, n_verlet_iters, n_verlet_capped, n_bad_scatter,
       n_analog_killed;
   double sum_w_emit, sum_w_rec, sum_w_horizon, sum_w_roulette_killed, sum_w_roulette_gain,
-      sum_w_outofrange, sum_w_maxstep, sum_w_absorbed, sum_wE_emit, sum_wE_rec, sum_w_bad;
+      sum_w_outofrange, sum_w_maxstep, sum_w_absorbed, sum_wE_emit, sum_wE_rec, sum_w_bad,
+      sum_w_spawned;   // total weight w/b handed to scattered superphotons; diagnostic of the Eq. 24-25 pin
 };
 struct Tally {
   std::vector<double> A, Q, W;  // sum wE, sum (wE)^2, sum w, per [n_th][n_nu]
@@ -170,6 +171,9 @@ double step_size(const Params& P, const double x[4], const double k[4]);
 void push_photon(const Params& P, const double x0[4], const double k0[4], const double a0[4], double dl,
                  double x1[4], double k1[4], double a1[4], int* iters, bool* capped);
 double bias_func(const Params& P, double thetae, int nsc);
+// fluid-frame photon energy eps = -k_mu u^mu (units m_e c^2) and cosine of the angle between the photon and
+// the magnetic field in that frame, (k.b)/(eps |b|) (all plasma quantities are fluid-frame)
+bool fluid_frame(const Context& C, const double k[4], const Geom& G, const Plasma& S, double* eps, double* cos_b);
 void opacities(const Context& C, const double x[4], const double k[4], const Geom& G, const Plasma& S,
                double* nua_a, double* nua_s, double* bias, int nsc);
 // Compton event (O8)

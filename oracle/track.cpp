@@ -11,7 +11,7 @@
 //                 photons are kept on an explicit stack (no recursion).
 //  record         detector binning; G26, G27.
 //
-// Pins (tests/test_oracle_track.py, test_oracle_sphere.py): straight lines in flat space,
+// Pins (tests/test_oracle_geometry.py, test_oracle_sphere.py, test_oracle_pins.py): straight lines in flat space,
 // E / L_z / Carter constant / k.k conservation in Kerr; absorbing uniform sphere closed form;
 // weight conservation with absorption off; bias-independence of the scattered spectrum;
 // N_s^-1/2 convergence.
@@ -71,23 +71,35 @@ double bias_func(const Params& P, double thetae, int nsc) {
   return b > 1.0 ? b : 1.0;
 }
 
+// eps = -k.u and cos(theta_B) = k.b/(eps |b|) in the fluid frame; false when eps is not a
+// positive finite number.  cos_b is 0 when the field vanishes.
+bool fluid_frame(const Context& C, const double k[4], const Geom& G, const Plasma& S, double* eps_out, double* cos_b) {
+  double kcov[4];
+  lower(G.gcov, k, kcov);
+  double eps = 0.0, kb = 0.0;
+  for (int m = 0; m < 4; m++) { eps -= kcov[m] * S.ucon[m]; kb += kcov[m] * S.bcon[m]; }
+  *eps_out = eps; *cos_b = 0.0;
+  if (!(eps > 0.0) || !std::isfinite(eps)) return false;
+  if (S.B > 0.0) {
+    double bnorm = S.B / C.un.B;
+    double c = kb / (eps * bnorm);
+    if (c > 1.0) c = 1.0;
+    if (c < -1.0) c = -1.0;
+    *cos_b = c;
+  }
+  return true;
+}
+
 void opacities(const Context& C, const double x[4], const double k[4], const Geom& G, const Plasma& S,
                double* nua_a, double* nua_s, double* bias, int nsc) {
   (void)x;
   *nua_a = 0.0; *nua_s = 0.0; *bias = 1.0;
   if (S.vacuum) return;
   const Params& P = C.P;
-  double kcov[4];
-  lower(G.gcov, k, kcov);
-  double eps = 0.0, kb = 0.0;
-  for (int m = 0; m < 4; m++) { eps -= kcov[m] * S.ucon[m]; kb += kcov[m] * S.bcon[m]; }
-  if (!(eps > 0.0) || !std::isfinite(eps)) return;
+  double eps, c;
+  if (!fluid_frame(C, k, G, S, &eps, &c)) return;
   double nu = eps * ME * CL * CL / HPL;
   if (S.thetae >= P.thetae_min && S.B > 0.0) {
-    double bnorm = S.B / C.un.B;
-    double c = kb / (eps * bnorm);
-    if (c > 1.0) c = 1.0;
-    if (c < -1.0) c = -1.0;
     double s = std::sqrt(1.0 - c * c);
     *nua_a = nu_alpha_abs(C.T, nu, S.ne, S.thetae, S.B, s);
   }
@@ -222,7 +234,7 @@ static void track_one(const Context& C, Photon p, std::vector<Photon>* stack, Ta
             opacities(C, c.x, c.k, Ge, Se, &c.nua_a, &c.nua_s, &c.bias, c.nsc);
             double kc[4]; lower(Ge.gcov, c.k, kc); c.E0 = -kc[0];
             stack->push_back(c);
-            st->n_spawned++;
+            st->n_spawned++; st->sum_w_spawned += wc;
           } else {
             st->n_bad_scatter++; st->sum_w_bad += wc;
           }
@@ -273,7 +285,7 @@ static void stats_add(Stats* a, const Stats& b) {
   a->sum_w_roulette_killed += b.sum_w_roulette_killed; a->sum_w_roulette_gain += b.sum_w_roulette_gain;
   a->sum_w_outofrange += b.sum_w_outofrange; a->sum_w_maxstep += b.sum_w_maxstep;
   a->sum_w_absorbed += b.sum_w_absorbed; a->sum_wE_emit += b.sum_wE_emit; a->sum_wE_rec += b.sum_wE_rec;
-  a->sum_w_bad += b.sum_w_bad;
+  a->sum_w_bad += b.sum_w_bad; a->sum_w_spawned += b.sum_w_spawned;
 }
 
 void run_range(Context* C, int64_t first, int64_t n, int nthreads) {

@@ -48,7 +48,8 @@ class Stats(C.Structure):
         "n_maxstep", "n_outofrange", "n_steps_total", "n_verlet_iters", "n_verlet_capped", "n_bad_scatter",
         "n_analog_killed")] + [(n, C.c_double) for n in (
         "sum_w_emit", "sum_w_rec", "sum_w_horizon", "sum_w_roulette_killed", "sum_w_roulette_gain",
-        "sum_w_outofrange", "sum_w_maxstep", "sum_w_absorbed", "sum_wE_emit", "sum_wE_rec", "sum_w_bad")]
+        "sum_w_outofrange", "sum_w_maxstep", "sum_w_absorbed", "sum_wE_emit", "sum_wE_rec", "sum_w_bad",
+        "sum_w_spawned")]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}
@@ -100,6 +101,7 @@ class OracleLib:
         L.orc_emit.argtypes = [C.c_void_p, C.c_int64, C.c_void_p]
         L.orc_trace.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
         L.orc_plasma_at.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.orc_fluid_frame.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]
         for f, n in (("orc_K2_direct", 1), ("orc_F_direct", 1), ("orc_sigma_kn", 1), ("orc_sigma_hot_direct", 2),
                      ("orc_K2_eval", 1), ("orc_F_eval", 1), ("orc_sigma_hot_eval", 2), ("orc_jnu", 5),
                      ("orc_jnu_integrated", 4), ("orc_nu_alpha_abs", 5)):
@@ -293,3 +295,9 @@ class Oracle:
         o = np.zeros(12)
         self.L.orc_plasma_at(self.h, _p(x), _p(o))
         return dict(ne=o[0], thetae=o[1], B=o[2], ucon=o[3:7].copy(), bcon=o[7:11].copy(), vacuum=bool(o[11]))
+
+    def fluid_frame(self, x, k, nsc=0):
+        x = np.ascontiguousarray(x, dtype=float); k = np.ascontiguousarray(k, dtype=float)
+        o = np.zeros(6)
+        self.L.orc_fluid_frame(self.h, _p(x), _p(k), nsc, _p(o))
+        return dict(eps=o[0], cos_b=o[1], nua_a=o[2], nua_s=o[3], bias=o[4], vacuum=bool(o[5]))
