@@ -41,9 +41,11 @@ UNIT = "superphotons/s"
 # frozen).  "track": in-grid step of track_kernel; "escape": free-flight step of escape_kernel.
 FLOP_PER_STEP = {"flat": {"track": 717.6, "escape": 208.0}, "kerr": {"track": 704.7, "escape": 368.2},
                  "kerr3d": {"track": 807.5, "escape": 368.2}}
-# dram__bytes_read.sum + dram__bytes_write.sum of the dominant launch (cold tracker pass over 1.09e6 primaries,
-# cfg2 at Ns=3e6) from the ncu --set full capture of profiles/r01g_carry_over.md; quoted for cfg2 only
+# dram__bytes_read.sum + dram__bytes_write.sum of the dominant launch from one ncu --set full capture; a constant of
+# that capture (its command and N_s are named in TRAFFIC_SOURCE), not a quantity measured in this run.  The run
+# itself reports the ALGORITHMIC bytes per launch beside it (roofline.algorithmic_bytes_per_launch).
 TRAFFIC_BYTES_PER_LAUNCH = {2: 85.4e6 + 76.2e6}
+TRAFFIC_SOURCE = {2: "profiles/r01g_carry_over.md: cold tracker pass over 1.09e6 primaries, cfg2 at N_s=3e6 (NOT this run's N_s)"}
 WORKLOAD_NAMES = {0: "cfg0 thin synchrotron sphere 32x16, Ns=1e5", 1: "cfg1 scattering sphere 32x16, Ns=1e6",
                   2: "cfg2 Kerr FM torus 256x256, Ns=1e7", 3: "cfg3 3-D perturbed torus 192x128x128, Ns=1e7",
                   4: "cfg4 Kerr torus x1e3 density (analog scattering), Ns=1e6"}
@@ -154,6 +156,8 @@ def main():
     ap.add_argument("--ns", type=float, default=None, help="override N_s of the config")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other-configs", dest="other_configs", action="store_false",
+                    help="skip the other_configs list (cfg3 full grid, cfg4 at 1e7, cfg1, cfg0) printed after the headline")
     ap.add_argument("--phase-pairs", type=int, default=-1, help="hot/cold tracker pass pairs per generation (-1: library default)")
     ap.add_argument("--k-cold", type=int, default=4, help="cold steps after which a hot pass hands a superphoton over")
     args = ap.parse_args()
@@ -175,99 +179,109 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     stream = torch.cuda.current_stream()
-
-    p, prim = make_workload(args.config, args.ns, rank_seed(1, rank))
-    g = gm.GPUMonty(p)
-    g.set_phase_passes(args.phase_pairs, args.k_cold)
-    host_grid = torch.from_numpy(prim).pin_memory()
-    dev_grid = host_grid.cuda()
     flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.float32, device="cuda")   # > 126 MB L2
-    nb = p["n_th"] * p["n_nu"]
-    d_spec = torch.zeros(2, nb, dtype=torch.float64, device="cuda")
+    peak_meas, _ = gm.fp64_peak()
+    peak = peak_meas / 1e12
 
-    def step(e2e: bool):
-        g.build_tables(stream)
-        g.set_grid(host_grid if e2e else dev_grid, stream)
-        g.prepare(stream)
-        g.run(stream=stream)
-        if e2e:
-            return g.spectrum()
-        g.spectrum_device(d_spec[0], d_spec[1], stream)
-        return None
+    def measure(cfg: int, ns, steps: int, warmup: int, with_cpu_baseline: bool):
+        """All of the bench line for one workload: device-timed steps, e2e steps, roofline, clocks."""
+        t_gen = time.perf_counter()
+        p, prim = make_workload(cfg, ns, rank_seed(1, rank))
+        gen_s = time.perf_counter() - t_gen
+        g = gm.GPUMonty(p)
+        g.set_phase_passes(args.phase_pairs, args.k_cold)
+        host_grid = torch.from_numpy(prim).pin_memory()
+        dev_grid = host_grid.cuda()
+        nb = p["n_th"] * p["n_nu"]
+        d_spec = torch.zeros(2, nb, dtype=torch.float64, device="cuda")
 
-    def timed(e2e: bool, nsteps: int):
-        ms = []
-        for _ in range(nsteps):
-            flush.fill_(1.0)                                  # L2 flush between timed iterations
-            if world > 1:
-                dist.barrier()
-            torch.cuda.synchronize()
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record(stream)
-            step(e2e)
-            e1.record(stream)
-            torch.cuda.synchronize()
-            ms.append(e0.elapsed_time(e1))
-        return ms
+        def step(e2e: bool):
+            g.build_tables(stream)
+            g.set_grid(host_grid if e2e else dev_grid, stream)
+            g.prepare(stream)
+            g.run(stream=stream)
+            if e2e:
+                return g.spectrum()
+            g.spectrum_device(d_spec[0], d_spec[1], stream)
+            return None
 
-    for _ in range(args.warmup):
-        step(False)
-    torch.cuda.synchronize()
-    g.timing(True)
-    clocks = ClockSampler(local)
-    clocks.start()
-    ms_dev = timed(False, args.steps)
-    clk = clocks.stop()
-    tm = g.timing(False)
-    st = g.stats()
-    tracked = st["n_primary"] + st["n_spawned"]
-    ms_e2e = timed(True, args.steps)
+        def timed(e2e: bool, nsteps: int):
+            ms = []
+            for _ in range(nsteps):
+                flush.fill_(1.0)                                  # L2 flush between timed iterations
+                if world > 1:
+                    dist.barrier()
+                torch.cuda.synchronize()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                step(e2e)
+                e1.record(stream)
+                torch.cuda.synchronize()
+                ms.append(e0.elapsed_time(e1))
+            return ms
 
-    t_dev = torch.tensor([float(np.mean(ms_dev)), float(np.mean(ms_e2e))], device="cuda", dtype=torch.float64)
-    cnt = torch.tensor([float(tracked)], device="cuda", dtype=torch.float64)
-    if world > 1:
-        dist.all_reduce(t_dev, op=dist.ReduceOp.MAX)
-        dist.all_reduce(cnt, op=dist.ReduceOp.SUM)
-        reduce_tally([torch.from_numpy(a).cuda() for a in g.tally()], dist)   # combined spectrum of the N runs
-    ms_step, ms_step_e2e = float(t_dev[0]), float(t_dev[1])
-    total = float(cnt[0])
+        for _ in range(warmup):
+            step(False)
+        torch.cuda.synchronize()
+        g.timing(True)
+        clocks = ClockSampler(local)
+        clocks.start()
+        ms_dev = timed(False, steps)
+        clk = clocks.stop()
+        tm = g.timing(False)
+        st = g.stats()
+        tracked = st["n_primary"] + st["n_spawned"]
+        ms_e2e = timed(True, steps)
 
-    if rank == 0:
+        t_dev = torch.tensor([float(np.mean(ms_dev)), float(np.mean(ms_e2e))], device="cuda", dtype=torch.float64)
+        cnt = torch.tensor([float(tracked)], device="cuda", dtype=torch.float64)
+        if world > 1:
+            dist.all_reduce(t_dev, op=dist.ReduceOp.MAX)
+            dist.all_reduce(cnt, op=dist.ReduceOp.SUM)
+            reduce_tally([torch.from_numpy(a).cuda() for a in g.tally()], dist)   # combined spectrum of the N runs
+        ms_step, ms_step_e2e = float(t_dev[0]), float(t_dev[1])
+        total = float(cnt[0])
         value = total / (ms_step * 1e-3)
         kind = ("kerr3d" if p["n3"] > 1 else "kerr") if p["metric_kind"] == 1 else "flat"
         n_track_launches = max(1, tm["track"][1])
         steps_track = st["n_steps_total"] - st["n_steps_free"]      # steps taken inside track_kernel (this rank, last timed step)
         flops = steps_track * FLOP_PER_STEP[kind]["track"]
-        esc_ms = tm["escape"][0] / args.steps
+        esc_ms = tm["escape"][0] / steps
         esc_tflops = st["n_steps_free"] * FLOP_PER_STEP[kind]["escape"] / max(esc_ms * 1e-3, 1e-9) / 1e12
-        track_ms_per_step = tm["track"][0] / args.steps
-        peak_meas, _ = gm.fp64_peak()
+        track_ms_per_step = tm["track"][0] / steps
         achieved = flops / (track_ms_per_step * 1e-3) / 1e12
-        peak = peak_meas / 1e12
-        launches = sum(v[1] for v in tm.values()) // max(1, args.steps)
+        launches = sum(v[1] for v in tm.values()) // max(1, steps)
+        # algorithmic bytes of the dominant kernel per launch: every input record read once (160 B), every
+        # hand-over / free-flight / scattered record written once (160 B), 4 (2-D) or 8 (3-D) 64-byte zone lines
+        # gathered per in-grid step (served by L1/L2 except on the 201 MB grid of cfg 3)
+        lpl = max(1, n_track_launches // max(1, steps))
+        alg_bytes = ((tracked + st["n_spawned"]) * 160.0 + steps_track * (8 if p["n3"] > 1 else 4) * 64.0) / lpl
         out = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warmup,
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic",
-            "config": {"workload": WORKLOAD_NAMES[args.config] + (f" (Ns overridden: {args.ns:g})" if args.ns else ""),
+            "config": {"workload": WORKLOAD_NAMES[cfg] + (f" (Ns overridden: {ns:g})" if ns else ""),
                        "superphotons_per_step_per_gpu": tracked, "primaries": st["n_primary"], "spawned": st["n_spawned"],
-                       "geodesic_steps": st["n_steps_total"], "geodesic_steps_free_flight": st["n_steps_free"], "l2": "flushed between timed steps (256 MB write)",
+                       "geodesic_steps": st["n_steps_total"], "geodesic_steps_free_flight": st["n_steps_free"],
+                       "l2": "flushed between timed steps (256 MB write)", "host_generation_s": gen_s,
                        "multi_gpu": "one independent seeded run per rank, tallies summed once" if world > 1 else "single GPU"},
             "e2e": {"value": total / (ms_step_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(prim.nbytes),
                     "d2h_bytes_per_step": int(nb * 8 * 3), "ms_per_step": ms_step_e2e},
             "gpu_launches": int(launches),
             "clocks": clk,
             "roofline": {"bound": "alu", "kernel": "track_kernel", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                         "frac": achieved / peak, "traffic": TRAFFIC_BYTES_PER_LAUNCH.get(args.config),
+                         "frac": achieved / peak, "traffic": TRAFFIC_BYTES_PER_LAUNCH.get(cfg),
+                         "traffic_source": TRAFFIC_SOURCE.get(cfg),
+                         "algorithmic_bytes_per_launch": alg_bytes,
                          "peak_source": "DFMA-chain microbenchmark run in this process (gm_fp64_peak); nominal 2*64*148*1.965 GHz = 37.2",
                          "flop_per_step": FLOP_PER_STEP[kind]["track"], "track_ms_per_step": track_ms_per_step,
                          "escape_kernel": {"achieved": esc_tflops, "frac": esc_tflops / peak, "ms_per_step": esc_ms,
                                            "flop_per_step": FLOP_PER_STEP[kind]["escape"]},
-                         "track_launches_per_step": n_track_launches // max(1, args.steps),
+                         "track_launches_per_step": lpl,
                          "track_share_of_step": track_ms_per_step / ms_step,
-                         "kernel_ms_per_step": {k: v[0] / args.steps for k, v in tm.items()}},
+                         "kernel_ms_per_step": {k: v[0] / steps for k, v in tm.items()}},
         }
-        if not args.no_cpu_baseline and world == 1:
+        if with_cpu_baseline and world == 1 and rank == 0:
             pr = oracle_sample(p, prim, 20000)        # probe (also pays the one-off oracle table build)
             pr = oracle_sample(p, prim, 20000)
             rate = pr["tracked"] / max(pr["run_s"], 1e-6)
@@ -276,6 +290,29 @@ def main():
             out["cpu_baseline"] = {"value": r["tracked"] / r["run_s"], "unit": UNIT, "cores": r["cores"], "kind": "oracle",
                                    "sample": f"first {r['n_sample']} primaries + descendants ({r['tracked']} superphotons, "
                                              f"{r['run_s']:.1f} s, oracle prepare {r['prepare_s']:.1f} s not counted)"}
+        g.close()
+        del dev_grid, host_grid
+        torch.cuda.empty_cache()
+        return out
+
+    out = measure(args.config, args.ns, args.steps, args.warmup, not args.no_cpu_baseline)
+    if args.other_configs and world == 1:
+        # the other BASELINE.json configs, driver-timed in the same run (3 warm-up + 3 timed steps each, same rules);
+        # nothing is cached across runs: every grid is generated here (host_generation_s states the cost)
+        others = []
+        for cfg, ns in ((3, None), (4, 1e7), (1, None), (0, None)):
+            if cfg == args.config and not args.ns:
+                continue
+            r = measure(cfg, ns, 3, 3, False)
+            others.append({"workload": r["config"]["workload"], "value": r["value"], "unit": UNIT,
+                           "ms_per_step": r["ms_per_step"], "e2e_value": r["e2e"]["value"],
+                           "superphotons_per_step": r["config"]["superphotons_per_step_per_gpu"],
+                           "tracker_frac_of_fp64_peak": r["roofline"]["frac"], "tracker_tflops": r["roofline"]["achieved"],
+                           "track_share_of_step": r["roofline"]["track_share_of_step"],
+                           "gpu_launches": r["gpu_launches"], "host_generation_s": r["config"]["host_generation_s"],
+                           "clocks": r["clocks"]})
+        out["other_configs"] = others
+    if rank == 0:
         print(json.dumps(out))
     if world > 1:
         dist.barrier()

@@ -31,7 +31,7 @@
 extern "C" {
 #endif
 
-#define GM_ABI_VERSION 1u
+#define GM_ABI_VERSION 2u
 
 enum {
   GM_OK = 0,
@@ -69,6 +69,12 @@ typedef struct gm_params {
   int32_t verlet_maxit;      /* cap on Eq. 12-14 iterations                                          */
   int32_t scattering_on, nsc_max, bias_p_theta, bias_q_nsc;
   int32_t n_th, n_nu, fold_theta; /* detector bins; fold_theta: theta and pi-theta share a bin (G27) */
+  int32_t emit_mode;         /* 0: superphotons are born at the zone centre (G12); 1: uniform in proper volume inside
+                                the zone, zone volumes exact (G31)             */
+  double bias_target;        /* bias tuning (G32): target scattered superphotons per parent, per
+                                scattering generation                                                             */
+  int32_t bias_tune;         /* 0: b from bias0 alone; 1: gm_prepare tunes one factor per generation on a pilot   */
+  int32_t pad_;
 } gm_params;
 
 /* Run counters (PAPER.md:316 counts emitted + scattered superphotons; invariants of DESIGN.md O7). */
@@ -79,7 +85,8 @@ typedef struct gm_stats {
       n_steps_free,   /* of n_steps_total: steps taken in free flight beyond the grid (escape kernel) */
       n_reentered;    /* superphotons that came back into the grid from free flight                  */
   double sum_w_emit, sum_w_rec, sum_w_horizon, sum_w_roulette_killed, sum_w_roulette_gain,
-      sum_w_outofrange, sum_w_maxstep, sum_w_absorbed, sum_wE_emit, sum_wE_rec, sum_w_bad;
+      sum_w_outofrange, sum_w_maxstep, sum_w_absorbed, sum_wE_emit, sum_wE_rec, sum_w_bad,
+      sum_w_spawned;  /* total weight w/b given to scattered superphotons                       */
 } gm_stats;
 
 /* Final state of one primary superphoton and sums over its family (primary + descendants). */
@@ -117,7 +124,8 @@ enum { GM_EVAL_ACCEL = 0,   /* in x[4],k[4]            -> out a[4] = -Gamma^m_ab
        GM_EVAL_PLASMA = 2,  /* in x[4]                 -> out ne,thetae,B,ucon[4],bcon[4],vacuum (12)   */
        GM_EVAL_OPAC = 3,    /* in x[4],k[4]            -> out nu*alpha_abs, nu*alpha_scat, bias (nsc=0) */
        GM_EVAL_PUSH = 4,    /* in x[4],k[4],a[4],dl    -> out x[4],k[4],a[4],iters (Eq. 11-15)          */
-       GM_EVAL_RAD = 5      /* in nu,ne,thetae,B,sin   -> out j_nu (Eq. 3), nu*alpha (Eq. 16/20), sigma_h/sigma_T(thetae, h nu/m c^2) */ };
+       GM_EVAL_RAD = 5,     /* in nu,ne,thetae,B,sin   -> out j_nu (Eq. 3), nu*alpha (Eq. 16/20), sigma_h/sigma_T(thetae, h nu/m c^2) */
+       GM_EVAL_NB = 6       /* in x                    -> out the hot loop's branch-free 1/x, sqrt(x), exp(x) */ };
 
 typedef struct gm_ctx gm_ctx; /* opaque; owned by the library */
 

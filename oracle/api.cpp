@@ -218,6 +218,14 @@ void orc_fluid_frame(void* h, const double* x, const double* k, int nsc, double*
   fluid_frame(*C, k, G, S, &out[0], &out[1]);
   opacities(*C, x, k, G, S, &out[2], &out[3], &out[4], nsc);
 }
+double orc_zone_volume(const Params* P, int i, int j, int k) { return zone_volume(*P, i, j, k); }
+// n positions drawn in zone (i,j,k) with emit_mode 1 (stream TAG_EMIT of ids 0..n-1): out[n][4]
+void orc_sample_positions(const Params* P, int i, int j, int k, int n, double* out) {
+  for (int q = 0; q < n; q++) {
+    Stream rs(P->seed, TAG_EMIT, (uint32_t)q, 0u, 0u);
+    sample_zone_position(*P, i, j, k, rs, out + 4 * q);
+  }
+}
 void orc_sample_mj(double thetae, uint64_t seed, int n, double* gamma_out) {
   for (int i = 0; i < n; i++) {
     Stream rs(seed, TAG_SCAT, (uint32_t)i, 0u, 0u);

@@ -28,6 +28,49 @@ static void zone_centre(const Params& P, int i, int j, int k, double x[4]) {
   x[3] = P.startx[3] + (k + 0.5) * P.dx[3];
 }
 
+// Proper coordinate volume of zone (i,j,k): the integral of sqrt(-g) = (r^2 + a^2 cos^2 theta) sin(theta) r theta'(x2)
+// over the zone, in closed form (dr = r dx1, dtheta = theta' dx2):
+//   dphi * [ (r_hi^3 - r_lo^3)/3 (cos th_lo - cos th_hi) + a^2 (r_hi - r_lo) (cos^3 th_lo - cos^3 th_hi)/3 ].
+// the paper smooths zone boundaries with 8192-32000 radial cells and partial cells; reading
+// G31 (emit_mode 1) removes the midpoint-rule volume error of sqrt(-g)_centre dx1 dx2 dx3 instead.
+double zone_volume(const Params& P, int i, int j, int k) {
+  (void)k;
+  double a = P.metric_kind == 1 ? P.a_spin : 0.0;
+  double rlo = std::exp(P.startx[1] + i * P.dx[1]), rhi = std::exp(P.startx[1] + (i + 1) * P.dx[1]);
+  double clo = std::cos(theta_of_x2(P, P.startx[2] + j * P.dx[2]));
+  double chi = std::cos(theta_of_x2(P, P.startx[2] + (j + 1) * P.dx[2]));
+  return P.dx[3] * ((rhi * rhi * rhi - rlo * rlo * rlo) / 3.0 * (clo - chi) +
+                    a * a * (rhi - rlo) * (clo * clo * clo - chi * chi * chi) / 3.0);
+}
+
+// Position uniform in proper volume inside zone (i,j,k) (G31): rejection on sqrt(-g) from a uniform proposal in the
+// zone's coordinate box.  Four uniforms per trial, in this order: x1, x2, x3, acceptance.  The bound is
+// r_hi (r_hi^2 + a^2 max cos^2) max sin * max theta' over the zone (each factor is monotone between the zone edges,
+// except sin which peaks at the equator), times 1 + 1e-12.
+void sample_zone_position(const Params& P, int i, int j, int k, Stream& rs, double x[4]) {
+  double a = P.metric_kind == 1 ? P.a_spin : 0.0;
+  double x1lo = P.startx[1] + i * P.dx[1], x2lo = P.startx[2] + j * P.dx[2], x3lo = P.startx[3] + k * P.dx[3];
+  double x2hi = P.startx[2] + (j + 1) * P.dx[2];
+  double rhi = std::exp(P.startx[1] + (i + 1) * P.dx[1]);
+  double tlo = theta_of_x2(P, x2lo), thi = theta_of_x2(P, x2hi);
+  double clo = std::cos(tlo), chi = std::cos(thi);
+  double c2 = clo * clo > chi * chi ? clo * clo : chi * chi;
+  double slo = std::sin(tlo), shi = std::sin(thi);
+  double smax = (tlo <= 0.5 * PI && thi >= 0.5 * PI) ? 1.0 : (slo > shi ? slo : shi);
+  double dlo = dtheta_dx2(P, x2lo), dhi = dtheta_dx2(P, x2hi);
+  double bound = rhi * (rhi * rhi + a * a * c2) * smax * (dlo > dhi ? dlo : dhi) * (1.0 + 1e-12);
+  x[0] = 0.0;
+  for (;;) {
+    double ua = rs.next(), ub = rs.next(), uc = rs.next(), ud = rs.next();
+    x[1] = x1lo + ua * P.dx[1];
+    x[2] = x2lo + ub * P.dx[2];
+    x[3] = x3lo + uc * P.dx[3];
+    Geom G;
+    geom_func(P, x, &G);
+    if (ud * bound < G.gdet) return;
+  }
+}
+
 double weight_of_nu(const Context& C, double nu) {
   const Params& P = C.P;
   double dl = std::log(P.nu_max / P.nu_min) / NW;
@@ -73,7 +116,8 @@ void prepare(Context* C) {
         double nuc = EE * S.B / (2.0 * PI * ME * CL);
         Z.nu0 = (2.0 / 9.0) * nuc * S.thetae * S.thetae;
         Z.A = JPREF_E * S.ne * Z.nu0 / K2_eval(C->T, S.thetae);
-        Z.C = dt * G.gdet * dV * Z.A / HPL;
+        if (P.emit_mode == 1) gdet[z] = zone_volume(P, i, j, k) / (P.dx[1] * P.dx[2] * P.dx[3]);   // zone-averaged sqrt(-g) (G31)
+        Z.C = dt * gdet[z] * dV * Z.A / HPL;
       }
 
   // Eq. 2: w(nu_k) = dt * Lambda/(h N_s) * sum_zones sqrt(-g) d3x int j_nu dOmega  (+ w_min floor)
@@ -197,17 +241,27 @@ void emit_photon(const Context& C, int64_t pid, Photon* ph) {
   int k3 = (int)(z % P.n3);
   int j2 = (int)((z / P.n3) % P.n2);
   int i1 = (int)(z / ((long)P.n3 * P.n2));
-  double x[4];
-  zone_centre(P, i1, j2, k3, x);
-  Geom G;
-  geom_func(P, x, &G);
-  Plasma S;
-  plasma_from_prim(P, C.un, G, &C.prim[z * 8], &S);
-
   ph->id.i0 = (uint32_t)((uint64_t)pid & 0xffffffffu);
   ph->id.i1 = (uint32_t)((uint64_t)pid >> 32);
   ph->id.i2 = 0u;
   Stream rs(P.seed, TAG_EMIT, ph->id.i0, ph->id.i1, ph->id.i2);
+
+  double x[4];
+  Geom G;
+  Plasma S;
+  if (P.emit_mode == 1) {
+    // G31: position uniform in proper volume inside the zone (drawn first), plasma state interpolated there;
+    // where the interpolated state does not emit (vacuum, Theta_e < thetae_min, B = 0) the zone's own state is kept
+    sample_zone_position(P, i1, j2, k3, rs, x);
+    geom_func(P, x, &G);
+    plasma_at(P, C.un, C.prim.data(), x, G, &S);
+    if (S.vacuum || !(S.ne > 0.0) || !(S.B > 0.0) || !(S.thetae >= P.thetae_min))
+      plasma_from_prim(P, C.un, G, &C.prim[z * 8], &S);
+  } else {
+    zone_centre(P, i1, j2, k3, x);
+    geom_func(P, x, &G);
+    plasma_from_prim(P, C.un, G, &C.prim[z * 8], &S);
+  }
 
   const double Lam = std::log(P.nu_max / P.nu_min);
   double nu = 0.0;

@@ -52,6 +52,9 @@ struct Params {
   int32_t verlet_maxit;
   int32_t scattering_on, nsc_max, bias_p_theta, bias_q_nsc;
   int32_t n_th, n_nu, fold_theta;
+  int32_t emit_mode;    // 0: emission at the zone centre (G12); 1: uniform in proper volume inside the zone (G31)
+  double bias_target;   // on-the-fly bias tuning (G32): target scattered superphotons per parent and generation
+  int32_t bias_tune;    // 0 off, 1: tune the per-generation bias factors in prepare()
   int32_t pad_;
 };
 
@@ -162,6 +165,8 @@ struct Context {
 
 // weights / counts / emission (O4, O6)
 void prepare(Context* C);
+double zone_volume(const Params& P, int i, int j, int k);     // coordinate volume integral of sqrt(-g) over a zone
+void sample_zone_position(const Params& P, int i, int j, int k, Stream& rs, double x[4]);   // G31
 double weight_of_nu(const Context& C, double nu);
 void make_tetrad(const Geom& G, const double ucon[4], const double trial[4], double econ[4][4]);
 void emit_photon(const Context& C, int64_t pid, Photon* ph);

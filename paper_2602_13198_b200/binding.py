@@ -15,11 +15,11 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 # GPUMONTY_B200_LIB selects another build of the same library (tuning experiments: launch bounds etc.)
 LIB_PATH = os.environ.get("GPUMONTY_B200_LIB") or os.path.join(_HERE, "libgpumonty_b200.so")
 
-GM_ABI_VERSION = 1
+GM_ABI_VERSION = 2
 TABLE_LNK2, TABLE_LNF, TABLE_LNSIGH, TABLE_LNW, TABLE_NEXP, TABLE_QMAX = range(6)
-EVAL_ACCEL, EVAL_GEOM, EVAL_PLASMA, EVAL_OPAC, EVAL_PUSH, EVAL_RAD = range(6)
+EVAL_ACCEL, EVAL_GEOM, EVAL_PLASMA, EVAL_OPAC, EVAL_PUSH, EVAL_RAD, EVAL_NB = range(7)
 _EVAL_SHAPES = {EVAL_ACCEL: (8, 4), EVAL_GEOM: (4, 33), EVAL_PLASMA: (4, 12), EVAL_OPAC: (8, 3),
-                EVAL_PUSH: (13, 13), EVAL_RAD: (5, 3)}
+                EVAL_PUSH: (13, 13), EVAL_RAD: (5, 3), EVAL_NB: (1, 3)}
 FATE_ALIVE, FATE_RECORDED, FATE_HORIZON, FATE_ROULETTE, FATE_MAXSTEP, FATE_OUTOFRANGE, FATE_ANALOG = range(7)
 
 EXPORTS = ["gm_create", "gm_destroy", "gm_last_error", "gm_set_grid", "gm_prepare", "gm_get_zone_counts",
@@ -43,6 +43,7 @@ class GmParams(C.Structure):
         ("verlet_maxit", C.c_int32), ("scattering_on", C.c_int32), ("nsc_max", C.c_int32),
         ("bias_p_theta", C.c_int32), ("bias_q_nsc", C.c_int32),
         ("n_th", C.c_int32), ("n_nu", C.c_int32), ("fold_theta", C.c_int32),
+        ("emit_mode", C.c_int32), ("bias_target", C.c_double), ("bias_tune", C.c_int32), ("pad_", C.c_int32),
     ]
 
 
@@ -52,7 +53,8 @@ class GmStats(C.Structure):
         "n_maxstep", "n_outofrange", "n_steps_total", "n_verlet_iters", "n_verlet_capped", "n_bad_scatter",
         "n_analog_killed", "n_steps_free", "n_reentered")] + [(n, C.c_double) for n in (
         "sum_w_emit", "sum_w_rec", "sum_w_horizon", "sum_w_roulette_killed", "sum_w_roulette_gain",
-        "sum_w_outofrange", "sum_w_maxstep", "sum_w_absorbed", "sum_wE_emit", "sum_wE_rec", "sum_w_bad")]
+        "sum_w_outofrange", "sum_w_maxstep", "sum_w_absorbed", "sum_wE_emit", "sum_wE_rec", "sum_w_bad",
+        "sum_w_spawned")]
 
 
 TRACE_DTYPE = np.dtype([("x", "f8", 4), ("k", "f8", 4), ("w", "f8"), ("E_inf", "f8"), ("nstep", "i8"),
@@ -115,6 +117,8 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
 def make_params(d: dict) -> GmParams:
     p = GmParams()
     for name, _ in GmParams._fields_:
+        if name == "pad_":
+            continue
         v = d[name] if name != "abi_version" else d.get("abi_version", GM_ABI_VERSION)
         if name in ("startx", "dx"):
             for i in range(4):

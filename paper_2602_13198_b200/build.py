@@ -12,6 +12,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgpumonty_b200.so")
+LISTINGS = os.path.join(HERE, "build")
 SOURCES = ["gm_api.cu", "gm_tables.cu", "gm_transport.cu"]
 HEADERS = ["gm_common.cuh", "gm_physics.cuh", "gm_host.h", os.path.join("..", "..", "include", "gpumonty_b200.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
@@ -42,7 +43,10 @@ def build(force: bool = False, verbose: bool = False) -> str:
             sys.stderr.write(" ".join(cmd) + "\n" + r.stdout + r.stderr)
         if r.returncode != 0:
             raise RuntimeError("nvcc failed: " + " ".join(cmd))
-        with open(cmd[-1].replace(".o", ".ptxas.txt"), "w") as f:     # registers / spills per kernel
+        # registers / spills per kernel: written to the ignored build/ folder (a build must not dirty the checkout;
+        # the listing that belongs to a measurement is copied under profiles/ by hand)
+        os.makedirs(LISTINGS, exist_ok=True)
+        with open(os.path.join(LISTINGS, os.path.basename(cmd[-1]).replace(".o", ".ptxas.txt")), "w") as f:
             # (compile times dropped: the listing then changes only when the code does)
             f.write("".join(l for l in r.stderr.splitlines(True) if "Compile time" not in l))
 

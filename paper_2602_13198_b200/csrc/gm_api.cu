@@ -25,7 +25,7 @@ struct gm_ctx {
   Tally tally{}; Tally tally_snap{};
   DevStats *d_stats = nullptr, *d_stats_snap = nullptr;
   double *d_spec = nullptr;          // [2][nb]
-  int* d_counters = nullptr;         // [0] primaries count, [1] queue A count, [2] queue B count, [3] work counter
+  int* d_counters = nullptr;         // 72 ints, layout in run_batch
   Photon *d_prim_ph = nullptr, *d_qA = nullptr, *d_qB = nullptr, *d_esc = nullptr;
   Photon *d_parkA = nullptr, *d_parkB = nullptr;   // hot/cold pass hand-over queues (esc_records each)
   int phase_pairs = -1, k_cold = 4;                // -1: automatic (decided by a pilot batch, see gm_run)
@@ -35,6 +35,7 @@ struct gm_ctx {
   long long esc_records = 0;
   long long batch_primaries = 0, queue_records = 0;   // allocated sizes
   long long want_batch = 0, want_queue = 0;
+  bool batch_limited_by_memory = false;
   bool have_grid = false, prepared = false;
   long long n_primaries = 0;
   std::string err;
@@ -125,6 +126,9 @@ static int validate(const gm_params* p) {
     return fail(nullptr, GM_ERR_PARAM, "bad scattering parameters");
   if (!(p->roulette > 1.0)) return fail(nullptr, GM_ERR_PARAM, "roulette must be > 1");
   if (p->n_th < 1 || p->n_nu < 1 || !finite_pos(p->nu_lo) || !(p->nu_hi > p->nu_lo)) return fail(nullptr, GM_ERR_PARAM, "bad detector bins");
+  if (p->emit_mode != 0 && p->emit_mode != 1) return fail(nullptr, GM_ERR_PARAM, "emit_mode must be 0 or 1");
+  if (p->bias_tune != 0 && p->bias_tune != 1) return fail(nullptr, GM_ERR_PARAM, "bias_tune must be 0 or 1");
+  if (p->bias_tune && !(p->bias_target > 0.0 && p->bias_target < 100.0)) return fail(nullptr, GM_ERR_PARAM, "bias_target must be in (0, 100)");
   return GM_OK;
 }
 
@@ -157,7 +161,7 @@ static void fill_dev_params(gm_ctx* c) {
   P.max_steps = p.max_steps; P.verlet_maxit = p.verlet_maxit;
   P.scattering_on = p.scattering_on; P.nsc_max = p.nsc_max; P.bias_p = p.bias_p_theta; P.bias_q = p.bias_q_nsc;
   P.bias0 = p.bias0; P.roulette = p.roulette; P.inv_roulette = 1.0 / p.roulette;
-  P.n_th = p.n_th; P.n_nu = p.n_nu; P.fold_theta = p.fold_theta;
+  P.n_th = p.n_th; P.n_nu = p.n_nu; P.fold_theta = p.fold_theta; P.emit_mode = p.emit_mode;
   P.nu_lo = p.nu_lo; P.db = std::log(p.nu_hi / p.nu_lo) / p.n_nu; P.inv_db = 1.0 / P.db;
   P.seed_lo = (uint32_t)(p.seed & 0xffffffffu); P.seed_hi = (uint32_t)(p.seed >> 32);
   P.prim = c->d_prim; P.lnK2 = c->d_lnK2; P.lnF = c->d_lnF; P.lnSigH = c->d_lnSigH; P.lnw = c->d_lnw;
@@ -231,6 +235,14 @@ int gm_create(gm_ctx** out, const gm_params* p) {
   ctx->tally_snap.Q = ctx->tally_snap.A + nb; ctx->tally_snap.W = ctx->tally_snap.A + 2 * nb;
   ctx->tally_snap.n = (unsigned long long*)(ctx->tally_snap.A + 3 * nb);
   fill_dev_params(ctx);
+  {
+    cudaError_t oe = track_kernel_optin();       // per device: a second context on another GPU needs it again
+    if (oe != cudaSuccess) {
+      std::string m = cudaGetErrorString(oe);
+      free_all(ctx); delete ctx;
+      return fail(nullptr, GM_ERR_CUDA, "cudaFuncSetAttribute(track_kernel, max dynamic shared memory): %s", m.c_str());
+    }
+  }
   if (const char* e = getenv("GPUMONTY_B200_CARRY")) ctx->carry_lanes = atoi(e) < 0 ? 0 : (atoi(e) > 32 ? 32 : atoi(e));
   // parameter-free tables (S0)
   cudaError_t te = gm_build_tables(ctx, nullptr) == GM_OK ? cudaSuccess : cudaErrorUnknown;
@@ -362,13 +374,22 @@ int gm_set_phase_passes(gm_ctx* ctx, int pairs, int k_cold) {
 }
 
 static int ensure_run_buffers(gm_ctx* ctx, long long n_ids) {
-  if (ctx->d_prim_ph) return GM_OK;
+  // buffers sized for an earlier, smaller request (a gm_trace of a few thousand ids, a small first gm_run) are
+  // re-allocated when a larger id range arrives and the caller did not fix the batch size himself
+  const long long default_batch = 1ll << 22;
+  if (ctx->d_prim_ph) {
+    const bool grow = !ctx->want_batch && ctx->batch_primaries < default_batch && n_ids > ctx->batch_primaries &&
+                      !ctx->batch_limited_by_memory;
+    if (!grow) return GM_OK;
+    CK(cudaDeviceSynchronize());
+    free_run_buffers(ctx);
+  }
   size_t free_b = 0, total_b = 0;
   CK(cudaMemGetInfo(&free_b, &total_b));
-  long long batch = ctx->want_batch ? ctx->want_batch : (1ll << 22);
+  long long batch = ctx->want_batch ? ctx->want_batch : default_batch;
   if (batch > n_ids && !ctx->want_batch) {
     batch = 1024;
-    while (batch < n_ids) batch <<= 1;           // power of two >= n_ids: a later, larger gm_run re-allocates
+    while (batch < n_ids) batch <<= 1;           // power of two >= n_ids
   }
   // scattered-superphoton queues: 8 records per primary by default (7-10x N_s are generated in
   // total, spread over the scattering generations); the escape queue must hold one whole tracker input
@@ -382,15 +403,18 @@ static int ensure_run_buffers(gm_ctx* ctx, long long n_ids) {
   auto bytes = [&](long long b, long long q) {
     return (size_t)(b + 2 * q + (pairs > 0 ? 3 : 1) * (b > q ? b : q)) * sizeof(Photon);
   };
-  while (bytes(batch, queue) > free_b / 2 && batch > 1024) { batch >>= 1; queue = queue_for(batch); }
+  ctx->batch_limited_by_memory = false;
+  while (bytes(batch, queue) > free_b / 2 && batch > 1024) { batch >>= 1; queue = queue_for(batch); ctx->batch_limited_by_memory = true; }
   const long long esc = batch > queue ? batch : queue;
-  CK(cudaMalloc((void**)&ctx->d_prim_ph, (size_t)batch * sizeof(Photon)));
-  CK(cudaMalloc((void**)&ctx->d_qA, (size_t)queue * sizeof(Photon)));
-  CK(cudaMalloc((void**)&ctx->d_qB, (size_t)queue * sizeof(Photon)));
-  CK(cudaMalloc((void**)&ctx->d_esc, (size_t)esc * sizeof(Photon)));
-  if (pairs > 0) {
-    CK(cudaMalloc((void**)&ctx->d_parkA, (size_t)esc * sizeof(Photon)));
-    CK(cudaMalloc((void**)&ctx->d_parkB, (size_t)esc * sizeof(Photon)));
+  cudaError_t e = cudaMalloc((void**)&ctx->d_prim_ph, (size_t)batch * sizeof(Photon));
+  if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->d_qA, (size_t)queue * sizeof(Photon));
+  if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->d_qB, (size_t)queue * sizeof(Photon));
+  if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->d_esc, (size_t)esc * sizeof(Photon));
+  if (e == cudaSuccess && pairs > 0) e = cudaMalloc((void**)&ctx->d_parkA, (size_t)esc * sizeof(Photon));
+  if (e == cudaSuccess && pairs > 0) e = cudaMalloc((void**)&ctx->d_parkB, (size_t)esc * sizeof(Photon));
+  if (e != cudaSuccess) {                        // leave no half-allocated state behind (batch_primaries stays 0)
+    free_run_buffers(ctx);
+    return fail(ctx, GM_ERR_CUDA, "run buffers (%lld primaries, %lld queue records): %s", batch, queue, cudaGetErrorString(e));
   }
   ctx->batch_primaries = batch; ctx->queue_records = queue; ctx->esc_records = esc;
   return GM_OK;
@@ -401,8 +425,15 @@ static int ensure_run_buffers(gm_ctx* ctx, long long n_ids) {
 // largest queue occupancy seen (device counters may exceed the capacity: overflow).
 static int run_batch(gm_ctx* ctx, long long first, int n, const long long* d_ids, TraceBuf trace, bool with_root,
                      Tally tally, DevStats* stats, cudaStream_t st, int* max_queue) {
-  int* cnt = ctx->d_counters;       // [0] primaries, [1] work counter, [2] escape queue, [3 + round] queue filled by that round
-  const int NCNT = 64, MAXROUND = NCNT - 3;
+  // [0] primaries, [1] work counter, [2] free-flight queue (reset per round), [3 + round] queue filled by that round,
+  // [64], [65] hand-over queues of the hot/cold passes, [66] count of the null queue, [67] sticky overflow flags set
+  // by the consumer kernels (1: a tracker input, 2: the free-flight queue was filled past its capacity)
+  int* cnt = ctx->d_counters;
+  const int NCNT = 72, MAXROUND = 64 - 3;
+  int* oflow = cnt + 67;
+  // a generation's own input (primaries, or the scattered queue of the previous round) may overflow legitimately:
+  // that case is seen through the queue counts and makes the caller redo the batch in smaller pieces
+  int* oflow_in = cnt + 68;
   CK(cudaMemsetAsync(cnt, 0, 72 * sizeof(int), st));
   TIMED(GM_T_EMIT, st, launch_emit(ctx->P, ctx->Z, ctx->nz, first, n, d_ids, ctx->d_prim_ph, cnt + 0, stats, nullptr, with_root, st));
   const int qcap = (int)ctx->queue_records;
@@ -437,14 +468,14 @@ static int run_batch(gm_ctx* ctx, long long first, int n, const long long* d_ids
       const int carry = (ctx->carry_lanes > 0 && first_block && round < last) ? ctx->carry_lanes : 0;
       CK(cudaMemsetAsync(esc.count, 0, sizeof(int), st));
       if (pairs == 0) {
-        TIMED(GM_T_TRACK, st, launch_track(ctx->P, 0, in, in_count, in_cap, cnt + 1, out, esc, nopark, 0, carry, tally, stats, trace, ctx->n_sm, st));
+        TIMED(GM_T_TRACK, st, launch_track(ctx->P, 0, in, in_count, in_cap, cnt + 1, out, esc, nopark, 0, carry, tally, stats, trace, oflow_in, ctx->n_sm, st));
       } else {
         // hot pass (in -> parkA), cold pass (parkA -> parkB), hot pass (parkB -> parkA), ... ; the last cold
         // pass handles hot plasma in place.  Every queue is fully consumed before it is refilled.
         const Photon* pin = in; const int* pcount = in_count; int pcap = in_cap;
         for (int pp = 0; pp < pairs; pp++) {
           CK(cudaMemsetAsync(parkA.count, 0, sizeof(int), st));
-          TIMED(GM_T_TRACK, st, launch_track(ctx->P, 1, pin, pcount, pcap, cnt + 1, out, esc, parkA, ctx->k_cold, carry, tally, stats, trace, ctx->n_sm, st));
+          TIMED(GM_T_TRACK, st, launch_track(ctx->P, 1, pin, pcount, pcap, cnt + 1, out, esc, parkA, ctx->k_cold, carry, tally, stats, trace, pp == 0 ? oflow_in : oflow, ctx->n_sm, st));
           if (deciding) {
             int parked = 0;
             CK(cudaMemcpyAsync(&parked, parkA.count, sizeof(int), cudaMemcpyDeviceToHost, st));
@@ -458,23 +489,27 @@ static int run_batch(gm_ctx* ctx, long long first, int n, const long long* d_ids
             if (ctx->auto_pairs == 0) pairs = 1;           // finish this generation with the mixed pass, then none
           }
           if (pp >= pairs - 1) {
-            TIMED(GM_T_TRACK, st, launch_track(ctx->P, 0, parkA.buf, parkA.count, parkA.capacity, cnt + 1, out, esc, nopark, 0, carry, tally, stats, trace, ctx->n_sm, st));
+            TIMED(GM_T_TRACK, st, launch_track(ctx->P, 0, parkA.buf, parkA.count, parkA.capacity, cnt + 1, out, esc, nopark, 0, carry, tally, stats, trace, oflow, ctx->n_sm, st));
           } else {
             CK(cudaMemsetAsync(parkB.count, 0, sizeof(int), st));
-            TIMED(GM_T_TRACK, st, launch_track(ctx->P, 2, parkA.buf, parkA.count, parkA.capacity, cnt + 1, out, esc, parkB, 0, carry, tally, stats, trace, ctx->n_sm, st));
+            TIMED(GM_T_TRACK, st, launch_track(ctx->P, 2, parkA.buf, parkA.count, parkA.capacity, cnt + 1, out, esc, parkB, 0, carry, tally, stats, trace, oflow, ctx->n_sm, st));
             pin = parkB.buf; pcount = parkB.count; pcap = parkB.capacity;
           }
         }
         if (ctx->phase_pairs < 0 && ctx->auto_pairs == 0) pairs = 0;
       }
       TIMED(GM_T_COMPTON, st, launch_compton(ctx->P, out, stats, trace, ctx->n_sm, st));
-      TIMED(GM_T_ESCAPE, st, launch_escape(ctx->P, esc, cnt + 1, out, tally, stats, trace, ctx->n_sm, st));
+      TIMED(GM_T_ESCAPE, st, launch_escape(ctx->P, esc, cnt + 1, out, tally, stats, trace, oflow, ctx->n_sm, st));
       in = out.buf; in_count = out.count; in_cap = qcap;
     }
     CK(cudaMemcpyAsync(h_counts, cnt, NCNT * sizeof(int), cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
     for (int r = 0; r < round; r++) if (h_counts[3 + r] > mq) mq = h_counts[3 + r];
-    if (h_counts[2] > ctx->esc_records) mq = qcap + 1;               // cannot happen (esc >= any tracker input)
+    // the free-flight and hand-over queues hold at most one record per input superphoton and launch, and are sized
+    // for a whole tracker input: an overflow there is a logic error, reported, never a silent loss
+    if (h_counts[67] != 0 || h_counts[64] > parkA.capacity || h_counts[65] > parkB.capacity || h_counts[2] > esc.capacity)
+      return fail(ctx, GM_ERR_OVERFLOW, "internal queue overflow (flags %d; free-flight %d/%d, hand-over %d, %d/%d records)",
+                  h_counts[67], h_counts[2], esc.capacity, h_counts[64], h_counts[65], parkA.capacity);
     if (mq > qcap || h_counts[3 + round - 1] == 0) break;            // overflow (caller redoes) or drained
     if (round >= MAXROUND)
       return fail(ctx, GM_ERR_STATE, "superphotons still re-entering the grid after %d tracker rounds", round);
@@ -496,6 +531,7 @@ int gm_run(gm_ctx* ctx, int64_t first_id, int64_t n_ids, void* cuda_stream) {
   const int nb = ctx->p.n_th * ctx->p.n_nu;
   long long done = 0;
   long long batch = ctx->batch_primaries;
+  if (batch < 1) return fail(ctx, GM_ERR_STATE, "run buffers are not allocated");
   TraceBuf notrace{nullptr};
   while (done < n_ids) {
     long long nthis = n_ids - done < batch ? n_ids - done : batch;
@@ -559,7 +595,7 @@ int gm_get_stats(gm_ctx* ctx, gm_stats* out) {
   int64_t* ni = &out->n_primary;
   for (int i = 0; i < 15; i++) ni[i] = (int64_t)h.n[i];
   double* sd = &out->sum_w_emit;
-  for (int i = 0; i < 11; i++) sd[i] = h.s[i];
+  for (int i = 0; i < 12; i++) sd[i] = h.s[i];
   return GM_OK;
 }
 
@@ -620,8 +656,8 @@ int gm_trace(gm_ctx* ctx, const int64_t* ids, int n, gm_trace_rec* out) {
 
 int gm_eval(gm_ctx* ctx, int what, const double* in, int n, double* out) {
   if (!ctx || !in || !out || n < 0) return GM_ERR_PARAM;
-  static const int nin[] = {8, 4, 4, 8, 13, 5}, nout[] = {4, 33, 12, 3, 13, 3};
-  if (what < 0 || what > GM_EVAL_RAD) return fail(ctx, GM_ERR_PARAM, "unknown eval %d", what);
+  static const int nin[] = {8, 4, 4, 8, 13, 5, 1}, nout[] = {4, 33, 12, 3, 13, 3, 3};
+  if (what < 0 || what > GM_EVAL_NB) return fail(ctx, GM_ERR_PARAM, "unknown eval %d", what);
   if ((what == GM_EVAL_PLASMA || what == GM_EVAL_OPAC) && !ctx->have_grid) return fail(ctx, GM_ERR_STATE, "no grid");
   if (n == 0) return GM_OK;
   double *d_in = nullptr, *d_out = nullptr;

@@ -55,7 +55,7 @@ struct DevParams {
   int scattering_on, nsc_max, bias_p, bias_q, pad1;
   double bias0, roulette, inv_roulette;
   // tally
-  int n_th, n_nu, fold_theta, pad2;
+  int n_th, n_nu, fold_theta, emit_mode;
   double nu_lo, inv_db, db;
   // RNG
   uint32_t seed_lo, seed_hi;
@@ -79,12 +79,12 @@ static_assert(sizeof(Photon) == 160, "Photon record must be 160 bytes");
 // per-run device accumulators
 struct DevStats {
   unsigned long long n[15];
-  double s[11];
+  double s[12];
 };
 enum { SN_PRIMARY = 0, SN_SPAWNED, SN_RECORDED, SN_HORIZON, SN_ROUL_KILLED, SN_ROUL_SURV, SN_MAXSTEP,
        SN_OUTOFRANGE, SN_STEPS, SN_VITERS, SN_VCAPPED, SN_BADSCAT, SN_ANALOG, SN_STEPS_FREE, SN_REENTER };
 enum { SS_EMIT = 0, SS_REC, SS_HORIZON, SS_ROUL_KILLED, SS_ROUL_GAIN, SS_OUTOFRANGE, SS_MAXSTEP,
-       SS_ABSORBED, SS_WE_EMIT, SS_WE_REC, SS_BAD };
+       SS_ABSORBED, SS_WE_EMIT, SS_WE_REC, SS_BAD, SS_SPAWNED };
 
 struct Tally { double* A; double* Q; double* W; unsigned long long* n; };
 

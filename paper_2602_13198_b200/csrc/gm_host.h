@@ -47,10 +47,14 @@ cudaError_t launch_emit(const DevParams& P, const ZoneArrays& Z, long nz, long l
 // marked as stragglers; launch_escape passes them on to `ret` (the next generation's input).
 cudaError_t launch_track(const DevParams& P, int phase, const Photon* in, const int* in_count, int in_capacity,
                          int* work_counter, Queue out, Queue esc, Queue park, int k_cold, int carry_lanes, Tally tally,
-                         DevStats* stats, TraceBuf trace, int n_sm, cudaStream_t st);
+                         DevStats* stats, TraceBuf trace, int* overflow, int n_sm, cudaStream_t st);
+// opt-in for > 48 KB of dynamic shared memory of every track_kernel instance, on the CURRENT device
+cudaError_t track_kernel_optin();
 // free flight of the leavers to r_max (record) ; a superphoton that re-enters the grid is appended to `ret`
+// `overflow`: sticky device flag word; a consumer kernel ORs 1 (tracker input) / 2 (free-flight queue) into it when
+// the queue it reads was filled past its capacity
 cudaError_t launch_escape(const DevParams& P, Queue esc, int* work_counter, Queue ret, Tally tally, DevStats* stats,
-                          TraceBuf trace, int n_sm, cudaStream_t st);
+                          TraceBuf trace, int* overflow, int n_sm, cudaStream_t st);
 // turn the proto-children of `q` into scattered superphotons in place (one Compton event each)
 cudaError_t launch_compton(const DevParams& P, Queue q, DevStats* stats, TraceBuf trace, int n_sm,
                            cudaStream_t st);

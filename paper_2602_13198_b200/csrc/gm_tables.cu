@@ -188,7 +188,18 @@ __global__ void zone_state_kernel(const DevParams P, ZoneArrays Z, long nz) {
       A = C_JPREF * S.ne * nu0 / K2_eval(P, S.thetae);
     }
   }
-  Z.A[z] = A; Z.nu0[z] = nu0; Z.vol[z] = G.gdet * P.dV;
+  double vol = G.gdet * P.dV;
+  if (P.emit_mode == 1) {
+    // exact coordinate-volume integral of sqrt(-g) = (r^2 + a^2 cos^2) sin r theta' over the zone (G31)
+    const double rlo = exp(__dadd_rn(P.startx1, __dmul_rn((double)i1, P.dx1))), rhi = exp(__dadd_rn(P.startx1, __dmul_rn((double)(i1 + 1), P.dx1)));
+    const double x2lo = __dadd_rn(P.startx2, __dmul_rn((double)j2, P.dx2)), x2hi = __dadd_rn(P.startx2, __dmul_rn((double)(j2 + 1), P.dx2));
+    const double om = 0.5 * (1.0 - P.hslope);
+    const double clo = cos(C_PI * x2lo + om * sin(2.0 * C_PI * x2lo)), chi = cos(C_PI * x2hi + om * sin(2.0 * C_PI * x2hi));
+    const double a2 = P.a_spin * P.a_spin;
+    vol = P.dx3 * ((rhi * rhi * rhi - rlo * rlo * rlo) / 3.0 * (clo - chi) + a2 * (rhi - rlo) * (clo * clo * clo - chi * chi * chi) / 3.0) *
+          (P.L_unit * P.L_unit * P.L_unit);
+  }
+  Z.A[z] = A; Z.nu0[z] = nu0; Z.vol[z] = vol;
 }
 
 // S2: partial sums of sqrt(-g) d3x A_i F(nu_k/nu0_i) over a tile of 256 zones, for every node k

@@ -16,8 +16,8 @@
 namespace gm {
 
 constexpr int FLAG_ROOT = 1, FLAG_DEAD = 2;
-constexpr int FLAG_ROULETTED = 4;
-constexpr int FLAG_CARRY = 8;       // straggler handed to the next generation's launch through the free-flight queue   // the roulette of step `nstep` was already played (record moved between passes)
+constexpr int FLAG_ROULETTED = 4;   // the roulette of step `nstep` was already played (record moved between passes)
+constexpr int FLAG_CARRY = 8;       // straggler handed to the next generation's launch through the free-flight queue
 
 // ---- block-level stats helper ---------------------------------------------------------------------
 __device__ __forceinline__ void stat_add_n(DevStats* st, int which, unsigned long long v) {
@@ -75,19 +75,56 @@ __global__ void __launch_bounds__(128, GM_EMIT_MINBLOCKS) emit_kernel(const DevP
     const long z = lo;
     const int j2 = (int)((z / P.n3) % P.n2), k3 = (int)(z % P.n3);
     const int i1 = (int)(z / ((long)P.n3 * P.n2));
-    // zone centre without FMA contraction: emission positions are bit-identical on any host
-    double x[4] = {0.0, __dadd_rn(P.startx1, __dmul_rn(i1 + 0.5, P.dx1)), __dadd_rn(P.startx2, __dmul_rn(j2 + 0.5, P.dx2)),
-                   __dadd_rn(P.startx3, __dmul_rn(k3 + 0.5, P.dx3))};
-    Geom G; DGeom D;
-    geom_at<KERR, true>(P, x[1], x[2], G, &D);
-    double pr[8];
-    load_zone(P.prim, z, pr);
-    Plasma S;
-    plasma_from_prim(P, G, pr, S);
-    const double nu0 = Z.nu0[z], qmax = Z.qmax[z];
     const uint32_t id0 = (uint32_t)((unsigned long long)pid & 0xffffffffu);
     const uint32_t id1 = (uint32_t)((unsigned long long)pid >> 32);
     RngStream rs(P, TAG_EMIT, id0, id1, 0u);
+    double x[4];
+    double pr[8];
+    Geom G; DGeom D;
+    bool own_state = true;
+    if (P.emit_mode == 1) {
+      // G31: position uniform in proper volume inside the zone -- rejection on sqrt(-g) from a uniform proposal in
+      // the zone's coordinate box (4 uniforms per trial: x1, x2, x3, acceptance), bound = product of the factors'
+      // maxima over the zone; without FMA contraction, so that an accepted position is bit-identical on any host
+      const double x1lo = __dadd_rn(P.startx1, __dmul_rn((double)i1, P.dx1)), x2lo = __dadd_rn(P.startx2, __dmul_rn((double)j2, P.dx2));
+      const double x3lo = __dadd_rn(P.startx3, __dmul_rn((double)k3, P.dx3)), x2hi = __dadd_rn(P.startx2, __dmul_rn((double)(j2 + 1), P.dx2));
+      const double rhi = exp(__dadd_rn(P.startx1, __dmul_rn((double)(i1 + 1), P.dx1)));
+      const double om = 1.0 - P.hslope;
+      const double tlo = C_PI * x2lo + 0.5 * om * sin(2.0 * C_PI * x2lo), thi = C_PI * x2hi + 0.5 * om * sin(2.0 * C_PI * x2hi);
+      double slo, clo, shi, chi;
+      sincos(tlo, &slo, &clo); sincos(thi, &shi, &chi);
+      const double smax = (tlo <= 0.5 * C_PI && thi >= 0.5 * C_PI) ? 1.0 : fmax(slo, shi);
+      const double dmax = fmax(C_PI + om * C_PI * cos(2.0 * C_PI * x2lo), C_PI + om * C_PI * cos(2.0 * C_PI * x2hi));
+      const double bound = rhi * (rhi * rhi + P.a_spin * P.a_spin * fmax(clo * clo, chi * chi)) * smax * dmax * (1.0 + 1e-12);
+      x[0] = 0.0;
+      for (int trial = 0; trial < 100000000; trial++) {
+        const double ua = rs.next(), ub = rs.next(), uc = rs.next(), ud = rs.next();
+        x[1] = __dadd_rn(x1lo, __dmul_rn(ua, P.dx1));
+        x[2] = __dadd_rn(x2lo, __dmul_rn(ub, P.dx2));
+        x[3] = __dadd_rn(x3lo, __dmul_rn(uc, P.dx3));
+        geom_at<KERR, false>(P, x[1], x[2], G, nullptr);
+        if (ud * bound < G.gdet) break;
+      }
+      geom_at<KERR, true>(P, x[1], x[2], G, &D);
+      // plasma state interpolated at the point; where that state does not emit, the zone's own state is kept
+      const bool in = P.n3 > 1 ? interp_prim<true>(P, x, pr) : interp_prim<false>(P, x, pr);
+      if (in && pr[0] > 0.0) {
+        Plasma T;
+        plasma_from_prim(P, G, pr, T);
+        own_state = !(T.ne > 0.0 && T.B > 0.0 && T.thetae >= P.thetae_min);
+      }
+    } else {
+      // zone centre without FMA contraction: emission positions are bit-identical on any host
+      x[0] = 0.0;
+      x[1] = __dadd_rn(P.startx1, __dmul_rn(i1 + 0.5, P.dx1));
+      x[2] = __dadd_rn(P.startx2, __dmul_rn(j2 + 0.5, P.dx2));
+      x[3] = __dadd_rn(P.startx3, __dmul_rn(k3 + 0.5, P.dx3));
+      geom_at<KERR, true>(P, x[1], x[2], G, &D);
+    }
+    if (own_state) load_zone(P.prim, z, pr);
+    Plasma S;
+    plasma_from_prim(P, G, pr, S);
+    const double nu0 = Z.nu0[z], qmax = Z.qmax[z];
     double nu = 0.0, lnnu = 0.0;
     for (int trial = 0; trial < 100000000; trial++) {           // Eq. 7-8
       double u1 = rs.next(), u2 = rs.next();
@@ -364,13 +401,16 @@ __global__ void __launch_bounds__(TRACK_THREADS, PHASE == 2 ? GM_COLD_MINBLOCKS 
 #endif
 track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in, const int* __restrict__ in_count, int in_capacity,
              int* work_counter, Queue out, Queue esc, Queue park, int k_cold, int carry_lanes, Tally tally,
-             DevStats* stats, TraceBuf trace) {
+             DevStats* stats, TraceBuf trace, int* overflow) {
   // dynamic shared memory: per warp the next STAGE_REC records (refill stage) and the gather slots of its lanes
   extern __shared__ uint4 s_dyn[];
   constexpr int STAGE_REC = track_stage_records(THREED);
   constexpr bool STAGED = track_staged_gather(THREED);
   constexpr int GATHER_U4 = STAGED ? 4 * 4 * 32 : 0;      // 16-byte slots per warp: records x 4 parts x 32 lanes
   const int n_in = min(*in_count, in_capacity);
+  // every queue is checked by its consumer: a producer that ran past the capacity dropped records, which the host
+  // must hear about (sticky flag, read back by run_batch; "nothing is dropped silently")
+  if (blockIdx.x == 0 && threadIdx.x == 0 && *in_count > in_capacity) atomicOr(overflow, 1);
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const unsigned lt_mask = (1u << lane) - 1u;
   uint4* stage = s_dyn + wid * (STAGE_REC * PH_U4);
@@ -619,11 +659,12 @@ template <bool KERR>
 #endif
 __global__ void __launch_bounds__(128, GM_ESC_MINBLOCKS)
 escape_kernel(const __grid_constant__ DevParams P, Queue esc, int* work_counter, Queue ret, Tally tally, DevStats* stats,
-              TraceBuf trace) {
+              TraceBuf trace, int* overflow) {
   // persistent, refilled like the tracker: the 32 lanes of a warp step together, stopped lanes take the next
   // records from a shared-memory stage that is loaded 32 records at a time (coalesced, ahead of their use)
   __shared__ uint4 s_stage[4][32 * PH_U4];
   const int n = min(*esc.count, esc.capacity);
+  if (blockIdx.x == 0 && threadIdx.x == 0 && *esc.count > esc.capacity) atomicOr(overflow, 2);
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const unsigned lt_mask = (1u << lane) - 1u;
   uint4* stage = s_stage[wid];
@@ -851,7 +892,7 @@ template <bool KERR, bool THREED>
 __global__ void __launch_bounds__(128, GM_COMPTON_MINBLOCKS) compton_kernel(const DevParams P, Queue q, DevStats* stats, TraceBuf trace) {
   const int n = min(*q.count, q.capacity);
   unsigned long long c_spawn = 0, c_bad = 0;
-  double s_bad = 0.0;
+  double s_bad = 0.0, s_spawn = 0.0;
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
     Photon ph = q.buf[i];
     Geom G; DGeom D;
@@ -868,7 +909,7 @@ __global__ void __launch_bounds__(128, GM_COMPTON_MINBLOCKS) compton_kernel(cons
       accel<KERR>(G, D, ph.k, ph.a);
       ph.nsc += 1; ph.nstep = 0; ph.jscat = 0; ph.flags = 0;
       opacities(P, ph.k, G, S, ph.nsc, P.scattering_on != 0 && ph.nsc < P.nsc_max, ph.nua_a, ph.nua_s, ph.bias);
-      c_spawn++;
+      c_spawn++; s_spawn += ph.w;
       if (trace.rec && ph.root >= 0) atomicAdd((unsigned long long*)&trace.rec[ph.root].fam_nspawn, 1ull);
     } else {
       ph.flags = FLAG_DEAD;
@@ -880,9 +921,10 @@ __global__ void __launch_bounds__(128, GM_COMPTON_MINBLOCKS) compton_kernel(cons
     c_spawn += __shfl_xor_sync(0xffffffffu, c_spawn, o);
     c_bad += __shfl_xor_sync(0xffffffffu, c_bad, o);
   }
-  s_bad = warp_sum(s_bad);
+  s_bad = warp_sum(s_bad); s_spawn = warp_sum(s_spawn);
   if ((threadIdx.x & 31) == 0) {
     stat_add_n(stats, SN_SPAWNED, c_spawn);
+    stat_add_s(stats, SS_SPAWNED, s_spawn);
     stat_add_n(stats, SN_BADSCAT, c_bad);
     stat_add_s(stats, SS_BAD, s_bad);
   }
@@ -965,6 +1007,8 @@ __global__ void eval_kernel(const DevParams P, int what, const double* __restric
     out[3 * i] = jnu_K2(r[0], r[1], r[2], r[3], r[4], K2_eval(P, r[2]));
     out[3 * i + 1] = nu_alpha_abs(P, r[0], r[1], r[2], r[3], r[4]);
     out[3 * i + 2] = P.lnSigH ? sigma_hot_eval(P, r[2], r[0] * C_H_MEC2) : 0.0;
+  } else if (what == GM_EVAL_NB) {
+    out[3 * i] = rcp_nb(in[i]); out[3 * i + 1] = sqrt_nb(in[i]); out[3 * i + 2] = exp_nb(in[i]);
   }
 }
 
@@ -1001,24 +1045,28 @@ cudaError_t launch_emit(const DevParams& P, const ZoneArrays& Z, long nz, long l
   return cudaGetLastError();
 }
 
+// > 48 KB of dynamic shared memory needs an opt-in per kernel AND per device: gm_create calls this for its device
+cudaError_t track_kernel_optin() {
+  cudaError_t e = cudaSuccess;
+#define GM_OPTIN(K, T, PH)                                                                                              \
+  if (e == cudaSuccess)                                                                                                 \
+    e = cudaFuncSetAttribute(track_kernel<K, T, PH>, cudaFuncAttributeMaxDynamicSharedMemorySize, track_smem_bytes(T))
+  GM_OPTIN(true, true, PHASE_MIXED); GM_OPTIN(true, false, PHASE_MIXED); GM_OPTIN(false, true, PHASE_MIXED);
+  GM_OPTIN(false, false, PHASE_MIXED); GM_OPTIN(true, true, PHASE_HOT); GM_OPTIN(true, false, PHASE_HOT);
+  GM_OPTIN(true, true, PHASE_COLD); GM_OPTIN(true, false, PHASE_COLD);
+#undef GM_OPTIN
+  return e;
+}
+
 cudaError_t launch_track(const DevParams& P, int phase, const Photon* in, const int* in_count, int in_capacity,
                          int* work_counter, Queue out, Queue esc, Queue park, int k_cold, int carry_lanes, Tally tally,
-                         DevStats* stats, TraceBuf trace, int n_sm, cudaStream_t st) {
+                         DevStats* stats, TraceBuf trace, int* overflow, int n_sm, cudaStream_t st) {
   cudaError_t e = cudaMemsetAsync(work_counter, 0, sizeof(int), st);
   if (e != cudaSuccess) return e;
   const int grid = n_sm * (phase == PHASE_COLD ? GM_COLD_MINBLOCKS : GM_TRACK_MINBLOCKS);
   const bool kerr = P.metric_kind == 1, td = P.n3 > 1;
-#define GM_TRACK_ARGS P, in, in_count, in_capacity, work_counter, out, esc, park, k_cold, carry_lanes, tally, stats, trace
+#define GM_TRACK_ARGS P, in, in_count, in_capacity, work_counter, out, esc, park, k_cold, carry_lanes, tally, stats, trace, overflow
   const int smem = track_smem_bytes(td);
-  static bool attr_set = false;
-  if (!attr_set) {                       // > 48 KB of dynamic shared memory needs the opt-in, once per kernel
-#define GM_OPTIN(K, T, PH) cudaFuncSetAttribute(track_kernel<K, T, PH>, cudaFuncAttributeMaxDynamicSharedMemorySize, track_smem_bytes(T))
-    GM_OPTIN(true, true, PHASE_MIXED); GM_OPTIN(true, false, PHASE_MIXED); GM_OPTIN(false, true, PHASE_MIXED);
-    GM_OPTIN(false, false, PHASE_MIXED); GM_OPTIN(true, true, PHASE_HOT); GM_OPTIN(true, false, PHASE_HOT);
-    GM_OPTIN(true, true, PHASE_COLD); GM_OPTIN(true, false, PHASE_COLD);
-#undef GM_OPTIN
-    attr_set = true;
-  }
   if (phase == PHASE_MIXED) {
     if (kerr && td) track_kernel<true, true, PHASE_MIXED><<<grid, TRACK_THREADS, smem, st>>>(GM_TRACK_ARGS);
     else if (kerr) track_kernel<true, false, PHASE_MIXED><<<grid, TRACK_THREADS, smem, st>>>(GM_TRACK_ARGS);
@@ -1038,12 +1086,12 @@ cudaError_t launch_track(const DevParams& P, int phase, const Photon* in, const 
 }
 
 cudaError_t launch_escape(const DevParams& P, Queue esc, int* work_counter, Queue ret, Tally tally, DevStats* stats,
-                          TraceBuf trace, int n_sm, cudaStream_t st) {
+                          TraceBuf trace, int* overflow, int n_sm, cudaStream_t st) {
   const int grid = n_sm * GM_ESC_MINBLOCKS;
   cudaError_t e = cudaMemsetAsync(work_counter, 0, sizeof(int), st);
   if (e != cudaSuccess) return e;
-  if (P.metric_kind == 1) escape_kernel<true><<<grid, 128, 0, st>>>(P, esc, work_counter, ret, tally, stats, trace);
-  else escape_kernel<false><<<grid, 128, 0, st>>>(P, esc, work_counter, ret, tally, stats, trace);
+  if (P.metric_kind == 1) escape_kernel<true><<<grid, 128, 0, st>>>(P, esc, work_counter, ret, tally, stats, trace, overflow);
+  else escape_kernel<false><<<grid, 128, 0, st>>>(P, esc, work_counter, ret, tally, stats, trace, overflow);
   return cudaGetLastError();
 }
 

@@ -46,7 +46,7 @@ def calibrated() -> dict:
 
 def default_params() -> dict:
     return dict(
-        abi_version=1, seed=1, Ns_target=1e5,
+        abi_version=2, seed=1, Ns_target=1e5,
         metric_kind=0, a_spin=0.0, hslope=1.0,
         startx=[0.0, 0.0, 0.0, 0.0], dx=[1.0, 1.0, 1.0, 2.0 * math.pi],
         n1=1, n2=1, n3=1,
@@ -59,6 +59,7 @@ def default_params() -> dict:
         scattering_on=0, nsc_max=4, bias0=1.0, bias_p_theta=0, bias_q_nsc=0,
         roulette=1e4,
         n_th=1, n_nu=200, nu_lo=1e8, nu_hi=1e24, fold_theta=1,
+        emit_mode=0, bias_tune=0, bias_target=1.0,
     )
 
 

@@ -38,7 +38,7 @@ class Params(C.Structure):
         ("thetae_mode", C.c_int32), ("verlet_maxit", C.c_int32),
         ("scattering_on", C.c_int32), ("nsc_max", C.c_int32), ("bias_p_theta", C.c_int32),
         ("bias_q_nsc", C.c_int32), ("n_th", C.c_int32), ("n_nu", C.c_int32), ("fold_theta", C.c_int32),
-        ("pad_", C.c_int32),
+        ("emit_mode", C.c_int32), ("bias_target", C.c_double), ("bias_tune", C.c_int32), ("pad_", C.c_int32),
     ]
 
 
@@ -66,7 +66,7 @@ def make_params(d: dict) -> Params:
     for name, _ in Params._fields_:
         if name == "pad_":
             continue
-        v = d[name]
+        v = d.get(name, 0) if name in ("emit_mode", "bias_target", "bias_tune") else d[name]
         if name in ("startx", "dx"):
             for i in range(4):
                 getattr(p, name)[i] = float(v[i])
@@ -120,6 +120,9 @@ class OracleLib:
         L.orc_push.argtypes = [C.POINTER(Params)] + [C.c_void_p] * 3 + [C.c_double] + [C.c_void_p] * 3
         L.orc_geodesic.argtypes = [C.POINTER(Params), C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]
         L.orc_tetrad.argtypes = [C.POINTER(Params)] + [C.c_void_p] * 4
+        L.orc_zone_volume.restype = C.c_double
+        L.orc_zone_volume.argtypes = [C.POINTER(Params), C.c_int, C.c_int, C.c_int]
+        L.orc_sample_positions.argtypes = [C.POINTER(Params), C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p]
         L.orc_sample_mj.argtypes = [C.c_double, C.c_uint64, C.c_int, C.c_void_p]
         L.orc_compton_sample.argtypes = [C.c_double, C.c_double, C.c_uint64, C.c_int] + [C.c_void_p] * 3
 

@@ -1,17 +1,19 @@
 """GPU parity tests proper: the CUDA path (through the C-ABI) against the CPU oracle, element by element, on the
 same seeded inputs and the same Philox streams (SURVEY.md 8(c) "History divergence").
 
-Tolerances (derived in DESIGN.md "Tolerances"):
+Tolerances (DESIGN.md section 3 "Tolerances of the GPU parity tests"):
   * integer / index work (Philox words, zone counts, prefix sum, bins, step counts): bit-exact;
   * device functions evaluated at the same point: 1e-11 relative (libdevice vs glibc last-ulp differences,
     closed-form vs generic-inverse metric algebra), tables 1e-9 (K2, F) / 3e-7 (sigma_h: the oracle's own
     quadrature tolerance is 1e-8);
   * per-history final state: |dw/w|, |dE/E| < 1e-7 for histories that did not fork; forked histories
     (a uniform within rounding of a threshold) must stay below 1e-3 of the sample;
-  * spectra: north_star's bar -- every bin holding >= 1000 superphotons within 1 % and within 3 sigma.
+  * spectra: north_star's bar -- every bin holding >= 1000 superphotons within 1 % and within 3 sigma; at full
+    size in tests/test_gpu_full_size.py, here on the bins above a stated lower count (their number asserted).
 """
 import ctypes
 import math
+import os
 
 import numpy as np
 import pytest
@@ -166,6 +168,38 @@ def test_radiation_functions(gm, olib):
         assert o_[2] == pytest.approx(sh, rel=1e-6)
 
 
+def test_branch_free_reciprocal_sqrt_exp_stay_within_one_ulp(gm):
+    """gm_physics.cuh replaces 1/x, sqrt and exp in the hot loop by branch-free Newton / polynomial versions and
+    claims <= 1 ulp on the operands met there (metric denominators, 1 + q, b.b, ln r, -tau_a).  Checked through
+    gm_eval against 80-bit long-double references over those ranges, both signs where they occur."""
+    p, prim = wl.config0(Ns=1e3)
+    g = gm.GPUMonty(p)
+    rng = np.random.default_rng(17)
+
+    def ulps(got, ref_ld):
+        ref = ref_ld.astype(np.float64)
+        return np.abs((got.astype(np.longdouble) - ref_ld) / np.spacing(np.abs(ref)).astype(np.longdouble)).astype(float)
+
+    n = 200000
+    x = 10.0 ** rng.uniform(-250, 250, n) * rng.choice([-1.0, 1.0], n)            # reciprocal: any normal operand
+    x = np.concatenate([x, rng.uniform(0.5, 4.0, n)])
+    out = g.eval(gm.EVAL_NB, x)
+    e_rcp = ulps(out[:, 0], 1.0 / x.astype(np.longdouble))
+    xs = np.concatenate([10.0 ** rng.uniform(-280, 280, n), 1.0 + 10.0 ** rng.uniform(-12, 8, n), rng.uniform(0, 4, n), [0.0]])
+    out = g.eval(gm.EVAL_NB, xs)
+    e_sqrt = ulps(out[:-1, 1], np.sqrt(xs[:-1].astype(np.longdouble)))
+    assert out[-1, 1] == 0.0                                                       # sqrt_nb(0) = 0
+    xe = np.concatenate([rng.uniform(-700, 700, n), rng.uniform(-5, 12, n), -10.0 ** rng.uniform(-18, 2.8, n)])
+    out = g.eval(gm.EVAL_NB, xe)
+    e_exp = ulps(out[:, 2], np.exp(xe.astype(np.longdouble)))
+    line = "max error in ulp: rcp_nb %.3f, sqrt_nb %.3f, exp_nb %.3f" % (e_rcp.max(), e_sqrt.max(), e_exp.max())
+    print("\n" + line)
+    if os.path.isdir("gpurun_out"):
+        with open(os.path.join("gpurun_out", "fork_rates.md"), "a") as f:
+            f.write(line + "\n")
+    assert e_rcp.max() <= 1.0 and e_sqrt.max() <= 1.0 and e_exp.max() <= 1.0, line
+
+
 # ---------------------------------------------------------------------------------------------------
 # S2-S5: weights, counts, prefix sum, emission
 # ---------------------------------------------------------------------------------------------------
@@ -216,29 +250,45 @@ def test_scan_ragged_tail_and_empty_zones(gm):
 # ---------------------------------------------------------------------------------------------------
 # S6-S12: histories and spectra
 # ---------------------------------------------------------------------------------------------------
-def _compare_traces(o, g, ids, fork_budget):
+def _compare_traces(o, g, ids, fork_budget, label=None):
+    """Same-stream histories one by one.  A history "forks" when a uniform falls within rounding of a threshold
+    (or libdevice and glibc differ in the last ulp of a transcendental): every integer of its final state is
+    compared, the forks are counted, printed and (on the GPU box) appended to gpurun_out/fork_rates.md; the budget
+    is a bound on that measured rate (<= 3x what profiles/r02_fork_rates.md records)."""
     tg = g.trace(ids)
     to, fam_wE, fam_n = o.trace(ids)
     same = (tg["fate"] == to["fate"]) & (tg["nstep"] == to["nstep"]) & (tg["inu"] == to["inu"]) & \
            (tg["ith"] == to["ith"]) & (tg["jscat"] == to["jscat"])
     forks = np.nonzero(~same)[0]
-    assert len(forks) <= fork_budget * len(ids) + 1, (len(forks), len(ids), forks[:10], tg[forks[:5]], to[forks[:5]])
     ok = np.nonzero(same)[0]
+    fsame = ok[tg["fam_nspawn"][ok] == fam_n[ok]]
+    line = "| %s | %d | %d | %.2e | %d | %.2e |" % (label or os.environ.get("PYTEST_CURRENT_TEST", "?").split("::")[-1].split(" ")[0],
+                                                  len(ids), len(forks), len(forks) / len(ids), len(ok) - len(fsame),
+                                                  (len(ok) - len(fsame)) / max(1, len(ok)))
+    print("\nfork rate " + line)
+    if os.path.isdir("gpurun_out"):
+        with open(os.path.join("gpurun_out", "fork_rates.md"), "a") as f:
+            f.write(line + "\n")
+    assert len(forks) <= fork_budget * len(ids) + 1, (len(forks), len(ids), forks[:10], tg[forks[:5]], to[forks[:5]])
     assert np.max(_relerr(tg["w"][ok], to["w"][ok])) < 1e-7
     rec = ok[to["fate"][ok] == 1]
     assert np.max(_relerr(tg["E_inf"][rec], to["E_inf"][rec])) < 1e-7
     assert np.max(np.abs(tg["x"][ok] - to["x"][ok])) < 1e-7
     # family sums: only compare where the spawn counts agree (a fork inside a child changes them)
-    fsame = ok[tg["fam_nspawn"][ok] == fam_n[ok]]
     assert len(fsame) >= (1 - 10 * fork_budget) * len(ok) - 1
     assert np.max(_relerr(tg["fam_wE"][fsame], fam_wE[fsame], floor=1e-300)) < 1e-6
     return len(forks)
 
 
-def _compare_spectra(o, g, min_count=1000):
+def _compare_spectra(o, g, min_count=1000, min_bins=1):
+    """north_star's bar on the bins holding >= min_count superphotons: within 1 % and within 3 sigma.  The number of
+    bins that entered is asserted (a comparison that selects nothing proves nothing); at the small N_s of these
+    tests few bins reach 1000, so they pass their own threshold -- the full-size criterion lives in
+    tests/test_gpu_full_size.py."""
     so, sigo, no = o.spectrum()
     sg, sigg, ng = g.spectrum()
     sel = (no >= min_count) & (so > 0)
+    assert sel.sum() >= min_bins, (int(sel.sum()), min_bins)
     assert np.array_equal(ng[sel], no[sel]) or np.max(np.abs(ng[sel] - no[sel])) <= 3
     rel = np.abs(sg[sel] / so[sel] - 1)
     assert np.all(rel < 0.01), rel.max()
@@ -265,8 +315,7 @@ def test_config0_thin_sphere(gm):
     o, g = _pair(gm, p, prim)
     o.run(); g.run()
     _compare_stats(o, g)
-    nb, worst = _compare_spectra(o, g, min_count=200)
-    assert nb >= 20
+    _compare_spectra(o, g, min_count=200, min_bins=20)
     A_o, Q_o, W_o, n_o = o.tally()
     A_g, Q_g, W_g, n_g = g.tally()
     assert np.array_equal(n_o, n_g)                       # every superphoton lands in the same bin
@@ -295,7 +344,7 @@ def test_config1_scattering_sphere_small(gm):
     so, sg = o.stats(), g.stats()
     assert sg["n_spawned"] > 5e3
     _compare_stats(o, g, rel=2e-3)
-    _compare_spectra(o, g, min_count=1000)
+    _compare_spectra(o, g, min_count=200, min_bins=15)
     ids = np.arange(0, g.n_primaries, 23)
     _compare_traces(o, g, ids, fork_budget=2e-3)
     # weight bookkeeping on the GPU
@@ -312,7 +361,7 @@ def test_config2_torus_small(gm):
     sg = g.stats()
     assert sg["n_spawned"] > 2 * sg["n_primary"] and sg["n_horizon"] > 0
     _compare_stats(o, g, rel=5e-3)
-    _compare_spectra(o, g, min_count=1000)
+    _compare_spectra(o, g, min_count=200, min_bins=60)
     ids = np.arange(0, g.n_primaries, 11)
     _compare_traces(o, g, ids, fork_budget=5e-3)
 
@@ -386,9 +435,46 @@ def test_partial_cell_sphere_boundary(gm, scattering):
     assert g.zone_counts().reshape(n1, 16)[n1 - 1].sum() == 0 and g.zone_counts().reshape(n1, 16)[n1 - 2].sum() > 0
     o.run(); g.run()
     _compare_stats(o, g, rel=1e-6)
-    _compare_spectra(o, g, min_count=300)
+    _compare_spectra(o, g, min_count=300, min_bins=10)
     ids = np.arange(0, g.n_primaries, 17)
     _compare_traces(o, g, ids, fork_budget=2e-3)
+
+
+@pytest.mark.parametrize("cfg", ["sphere", "torus3d"])
+def test_subzone_emission_positions(gm, cfg):
+    """emit_mode = 1 (G31): exact zone volumes, superphotons born uniformly in proper volume
+    inside their zone (rejection on sqrt(-g), 4 uniforms per trial drawn before the frequency trials), plasma state
+    interpolated at the point.  Counts bit-exact, positions bit-equal (a rejection decision within rounding of its
+    threshold would show as a fork), histories and spectrum against the oracle."""
+    if cfg == "sphere":
+        p, prim = wl.config0(emit_mode=1)
+    else:
+        p, prim = wl.config3(Ns=1e4, n1=48, n2=32, n3=32, emit_mode=1)
+    o, g = _pair(gm, p, prim)
+    assert np.array_equal(o.zone_counts(), g.zone_counts())
+    assert np.max(_relerr(o.zone_info()[0], g.table(gm.TABLE_NEXP))) < 1e-11
+    ids = np.unique(np.random.default_rng(8).integers(0, g.n_primaries, 800))
+    eg = g.emit(ids)
+    nx = 0
+    for i, rec in zip(ids, eg):
+        r = o.emit(int(i))
+        if not np.array_equal(rec["x"], r["x"]):
+            nx += 1
+            continue
+        assert np.max(np.abs(rec["k"] - r["k"])) < 1e-10 * np.max(np.abs(r["k"])), (i, rec["k"], r["k"])
+        assert rec["w"] == pytest.approx(r["w"], rel=1e-10)
+        assert rec["nua_a"] == pytest.approx(r["nua_a"], rel=1e-9, abs=1e-300)
+        assert rec["E0"] == pytest.approx(r["E0"], rel=1e-10)
+    assert nx <= 1, nx
+    # the positions really are spread over the zones
+    x1 = (eg["x"][:, 1] - p["startx"][1]) / p["dx"][1]
+    assert 0.2 < np.std(x1 - np.floor(x1)) < 0.35
+    o.run(); g.run()
+    _compare_stats(o, g, rel=5e-3 if cfg != "sphere" else 1e-6)
+    if cfg == "sphere":
+        _compare_spectra(o, g, min_count=200, min_bins=20)
+        assert np.array_equal(o.tally()[3], g.tally()[3])
+    _compare_traces(o, g, np.arange(0, g.n_primaries, 11), fork_budget=5e-3)
 
 
 @pytest.mark.parametrize("cfg,pairs,k_cold", [(2, 1, 1), (2, 2, 4), (2, 3, 2), (3, 2, 3), (4, 2, 1)])
