@@ -218,7 +218,10 @@ __host__ __device__ constexpr bool track_staged_gather(bool) { return false; }
 #else
 __host__ __device__ constexpr bool track_staged_gather(bool threed) { return !threed; }
 #endif
-__host__ __device__ constexpr int track_stage_records(bool) { return 32; }
+#ifndef GM_STAGE_REC
+#define GM_STAGE_REC 32
+#endif
+__host__ __device__ constexpr int track_stage_records(bool) { return GM_STAGE_REC; }
 __host__ __device__ constexpr int track_smem_bytes(bool threed) {
   return TRACK_WARPS * (track_stage_records(threed) * PH_U4 + (track_staged_gather(threed) ? 4 * 4 * 32 : 0)) * 16;
 }
@@ -493,18 +496,12 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
       double ur;
       uniform_pair(P, TAG_STEP, L.id0, L.id1, L.id2, L.nstep, ux, ur);
       if (L.w < P.w_min && !(L.flags & FLAG_ROULETTED)) {
-#ifdef GM_ROUL_CALL
-        const Lane T = L;
-        L.w = roulette(P, T, ur, stats, trace);
-        if (L.w < 0.0) { have = false; continue; }
-#else
         // most roulettes kill (survival 1/roulette): counted in registers, no call and no lane copy unless a
         // trace buffer wants the record
         if (ur >= P.inv_roulette && !trace.rec) { c_rk++; c_rkw += L.w; have = false; continue; }
         const Lane T = L;
         L.w = roulette(P, T, ur, stats, trace);
         if (L.w < 0.0) { have = false; continue; }
-#endif
         L.flags |= FLAG_ROULETTED;                        // cleared when the step is committed
       }
       dl = step_size(P, L.x, L.k);
