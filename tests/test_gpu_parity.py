@@ -323,7 +323,7 @@ def test_config0_thin_sphere(gm):
     assert np.max(_relerr(A_o[m], A_g[m])) < 1e-8
     assert np.max(_relerr(Q_o[m], Q_g[m])) < 1e-8
     ids = np.arange(0, g.n_primaries, 37)
-    _compare_traces(o, g, ids, fork_budget=1e-3)
+    _compare_traces(o, g, ids, fork_budget=2e-4)
 
 
 def test_scattering_off_reproduces_config0_path_bitwise(gm):
@@ -346,7 +346,7 @@ def test_config1_scattering_sphere_small(gm):
     _compare_stats(o, g, rel=2e-3)
     _compare_spectra(o, g, min_count=200, min_bins=15)
     ids = np.arange(0, g.n_primaries, 23)
-    _compare_traces(o, g, ids, fork_budget=2e-3)
+    _compare_traces(o, g, ids, fork_budget=2e-4)
     # weight bookkeeping on the GPU
     out = (sg["sum_w_rec"] + sg["sum_w_horizon"] + sg["sum_w_roulette_killed"] - sg["sum_w_roulette_gain"] +
            sg["sum_w_outofrange"] + sg["sum_w_maxstep"] + sg["sum_w_absorbed"] + sg["sum_w_bad"])
@@ -363,7 +363,7 @@ def test_config2_torus_small(gm):
     _compare_stats(o, g, rel=5e-3)
     _compare_spectra(o, g, min_count=200, min_bins=60)
     ids = np.arange(0, g.n_primaries, 11)
-    _compare_traces(o, g, ids, fork_budget=5e-3)
+    _compare_traces(o, g, ids, fork_budget=2e-4)
 
 
 def test_config3_3d_small(gm):
@@ -374,7 +374,7 @@ def test_config3_3d_small(gm):
     o.run(); g.run()
     _compare_stats(o, g, rel=5e-3)
     ids = np.arange(0, g.n_primaries, 7)
-    _compare_traces(o, g, ids, fork_budget=5e-3)
+    _compare_traces(o, g, ids, fork_budget=2e-4)
 
 
 def test_config4_analog_scattering_small(gm):
@@ -386,7 +386,7 @@ def test_config4_analog_scattering_small(gm):
     assert sg["n_analog_killed"] > 0
     _compare_stats(o, g, rel=5e-3)
     ids = np.arange(0, g.n_primaries, 5)
-    _compare_traces(o, g, ids, fork_budget=5e-3)
+    _compare_traces(o, g, ids, fork_budget=2e-4)
 
 
 @pytest.mark.parametrize("cfg", [1, 2])
@@ -437,7 +437,7 @@ def test_partial_cell_sphere_boundary(gm, scattering):
     _compare_stats(o, g, rel=1e-6)
     _compare_spectra(o, g, min_count=300, min_bins=10)
     ids = np.arange(0, g.n_primaries, 17)
-    _compare_traces(o, g, ids, fork_budget=2e-3)
+    _compare_traces(o, g, ids, fork_budget=2e-4)
 
 
 @pytest.mark.parametrize("cfg", ["sphere", "torus3d"])
@@ -474,7 +474,7 @@ def test_subzone_emission_positions(gm, cfg):
     if cfg == "sphere":
         _compare_spectra(o, g, min_count=200, min_bins=20)
         assert np.array_equal(o.tally()[3], g.tally()[3])
-    _compare_traces(o, g, np.arange(0, g.n_primaries, 11), fork_budget=5e-3)
+    _compare_traces(o, g, np.arange(0, g.n_primaries, 11), fork_budget=2e-4)
 
 
 @pytest.mark.parametrize("cfg,pairs,k_cold", [(2, 1, 1), (2, 2, 4), (2, 3, 2), (3, 2, 3), (4, 2, 1)])
@@ -549,7 +549,7 @@ def test_superphotons_reentering_the_grid_from_free_flight(gm, scattering):
         assert tm["track"][1] > 1
     _compare_stats(o, g, rel=5e-3)
     ids = np.arange(0, g.n_primaries, 3)
-    _compare_traces(o, g, ids, fork_budget=5e-3)
+    _compare_traces(o, g, ids, fork_budget=2e-4)
 
 
 def _full_size_checks(gm, p, prim, n_sample, seed):
@@ -572,7 +572,7 @@ def _full_size_checks(gm, p, prim, n_sample, seed):
            sg["sum_w_outofrange"] + sg["sum_w_maxstep"] + sg["sum_w_absorbed"] + sg["sum_w_bad"])
     assert out == pytest.approx(sg["sum_w_emit"], rel=1e-9)
     ids = np.sort(np.random.default_rng(seed).choice(g.n_primaries, n_sample, replace=False))
-    _compare_traces(o, g, ids, fork_budget=5e-3)
+    _compare_traces(o, g, ids, fork_budget=2e-4)
     return sg
 
 
@@ -602,6 +602,56 @@ def test_batching_and_queue_overflow_recovery(gm):
     assert np.array_equal(ref[3], got[3])
     assert np.max(_relerr(ref[0], got[0], floor=1e-300)) < 1e-12
     assert st["n_spawned"] == ref_stats["n_spawned"] and st["n_primary"] == ref_stats["n_primary"]
+
+
+@pytest.mark.parametrize("cfg,world", [(1, 2), (2, 3)])
+def test_contexts_on_disjoint_id_ranges_sum_to_the_single_run(gm, cfg, world):
+    """The multi-GPU code path of DESIGN.md section 10 on one device: `world` library contexts,
+    each tracking the contiguous primary-id range shard.id_range gives its rank (children stay with their root),
+    must add up to the single run: counts and counters exactly, sums to rounding (the order of fp64 atomics)."""
+    from paper_2602_13198_b200.shard import id_range
+    p, prim = (wl.config1(Ns=1e5) if cfg == 1 else wl.config2(Ns=3e4))
+    g = gm.GPUMonty(p); g.set_grid(prim); n = g.prepare(); g.run()
+    ref, ref_st = g.tally(), g.stats()
+    ctxs = []
+    for rank in range(world):                       # all contexts alive at once, as they would be on `world` GPUs
+        gi = gm.GPUMonty(p); gi.set_grid(prim)
+        assert gi.prepare() == n
+        ctxs.append(gi)
+    acc, st_acc, covered = None, None, 0
+    for rank, gi in enumerate(ctxs):
+        first, cnt = id_range(n, rank, world)
+        assert first == covered
+        covered += cnt
+        gi.run(first, cnt)
+        t, st = gi.tally(), gi.stats()
+        assert st["n_primary"] == cnt
+        acc = [a.copy() for a in t] if acc is None else [a + b for a, b in zip(acc, t)]
+        st_acc = dict(st) if st_acc is None else {k: st_acc[k] + v for k, v in st.items()}
+    assert covered == n
+    assert np.array_equal(acc[3], ref[3])
+    for a, b in zip(acc[:3], ref[:3]):
+        assert np.max(_relerr(a, b, floor=1e-300)) < 1e-12
+    for k, v in ref_st.items():
+        if k.startswith("n_"):
+            assert st_acc[k] == v, (k, st_acc[k], v)
+        else:
+            assert st_acc[k] == pytest.approx(v, rel=1e-11, abs=1e-300), k
+
+
+def test_small_first_request_does_not_pin_the_batch_size(gm):
+    """a small gm_trace / gm_run used to fix the internal batch at its own size, so that a later
+    full-size gm_run was cut into thousands of tiny batches.  The buffers are re-sized now: the large run after a
+    small one launches no more kernels than the large run alone."""
+    p, prim = wl.config1(Ns=3e5)
+    g1 = gm.GPUMonty(p); g1.set_grid(prim); n = g1.prepare()
+    g1.timing(True); g1.run(); t1 = g1.timing(False)
+    g2 = gm.GPUMonty(p); g2.set_grid(prim); g2.prepare()
+    g2.trace(np.arange(100))                       # allocates run buffers for 1024 primaries
+    g2.run(0, 500); g2.reset_tally()
+    g2.timing(True); g2.run(); t2 = g2.timing(False)
+    assert t2["track"][1] <= t1["track"][1] + 2, (t1["track"], t2["track"])
+    assert np.array_equal(g1.tally()[3], g2.tally()[3])
 
 
 def test_empty_and_degenerate_inputs(gm):
