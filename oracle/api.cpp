@@ -1,6 +1,7 @@
 // ORACLE (test infrastructure).  C entry points used by tests/, smoke() and bench.py's
 // cpu_baseline / --impl reference legs through ctypes (tests/oracle_binding.py).
 #include "oracle.hpp"
+#include <algorithm>
 #include <cmath>
 #include <cstring>
 #include <mutex>
@@ -39,7 +40,19 @@ int orc_prepare(void* h, int64_t* n_primaries) {
   ensure_tables(C->P.scattering_on != 0);
   C->T = g_tables;
   prepare(C);
+  if (C->P.bias_tune) tune_bias(C, omp_get_max_threads());     // G32: pilot on the first primaries, factors frozen after
   if (n_primaries) *n_primaries = C->offset.back();
+  return 0;
+}
+// per-generation bias factors (G32) and spawn counts since the last reset: 64 entries each
+int orc_get_bias_table(void* h, double* fac, int64_t* gen_spawn) {
+  Context* C = (Context*)h;
+  for (int g = 0; g < 64; g++) { if (fac) fac[g] = C->bias_fac[g]; if (gen_spawn) gen_spawn[g] = C->gen_spawn[g]; }
+  return C->tune_iterations;
+}
+int orc_set_bias_table(void* h, const double* fac) {
+  Context* C = (Context*)h;
+  for (int g = 0; g < 64; g++) C->bias_fac[g] = fac[g];
   return 0;
 }
 int orc_get_zone_counts(void* h, int32_t* out) {
@@ -68,6 +81,7 @@ int orc_reset_tally(void* h) {
   Context* C = (Context*)h;
   tally_init(C->P, &C->tally);
   C->stats = Stats();
+  std::fill(C->gen_spawn.begin(), C->gen_spawn.end(), 0);
   return 0;
 }
 int orc_get_tally(void* h, double* A, double* Q, double* W, int64_t* n) {

@@ -156,6 +156,8 @@ void prepare(Context* C) {
   }
   tally_init(P, &C->tally);
   C->stats = Stats();
+  std::fill(C->gen_spawn.begin(), C->gen_spawn.end(), 0);
+  std::fill(C->bias_fac.begin(), C->bias_fac.end(), 1.0);
   C->prepared = true;
 }
 

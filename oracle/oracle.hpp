@@ -160,8 +160,14 @@ struct Context {
   std::vector<ZoneInfo> zones;
   std::vector<int64_t> offset;          // exclusive scan of zone counts, size zones+1
   Tally tally; Stats stats;
+  // on-the-fly bias tuning (G32): one factor per scattering generation multiplying bias0, and the number of
+  // scattered superphotons each generation has spawned (index = n_sc of the parent) since the last reset
+  std::vector<double> bias_fac = std::vector<double>(64, 1.0);
+  std::vector<int64_t> gen_spawn = std::vector<int64_t>(64, 0);
+  int tune_iterations = 0;
   bool prepared = false;
 };
+void tune_bias(Context* C, int nthreads);
 
 // weights / counts / emission (O4, O6)
 void prepare(Context* C);
@@ -175,7 +181,7 @@ void emit_photon(const Context& C, int64_t pid, Photon* ph);
 double step_size(const Params& P, const double x[4], const double k[4]);
 void push_photon(const Params& P, const double x0[4], const double k0[4], const double a0[4], double dl,
                  double x1[4], double k1[4], double a1[4], int* iters, bool* capped);
-double bias_func(const Params& P, double thetae, int nsc);
+double bias_func(const Params& P, double thetae, int nsc, double fac = 1.0);
 // fluid-frame photon energy eps = -k_mu u^mu (units m_e c^2) and cosine of the angle between the photon and
 // the magnetic field in that frame, (k.b)/(eps |b|) (all plasma quantities are fluid-frame)
 bool fluid_frame(const Context& C, const double k[4], const Geom& G, const Plasma& S, double* eps, double* cos_b);
@@ -186,7 +192,7 @@ bool compton_event(const Context& C, const Photon& parent_at_event, const Geom& 
                    uint32_t j, double kout[4]);
 void sample_electron_mj(Stream& rs, double thetae, double* gamma_e, double* beta_e);  // for pins
 // history driver: tracks photon and all its descendants; tallies
-void track_history(const Context& C, Photon ph, Tally* tl, Stats* st, TraceRec* root_trace);
+void track_history(const Context& C, Photon ph, Tally* tl, Stats* st, TraceRec* root_trace, int64_t* gen_spawn = nullptr);
 void tally_init(const Params& P, Tally* tl);
 void run_range(Context* C, int64_t first, int64_t n, int nthreads);
 

@@ -16,6 +16,7 @@
 // weight conservation with absorption off; bias-independence of the scattered spectrum;
 // N_s^-1/2 convergence.
 #include "oracle.hpp"
+#include <algorithm>
 #include <cmath>
 #include <vector>
 #include <omp.h>
@@ -63,9 +64,10 @@ void push_photon(const Params& P, const double x0[4], const double k0[4], const 
   *capped = !conv;
 }
 
-// [parity unpinned] G21: b = max(1, bias0 * Theta_e^p * (n_sc+1)^q), integer p, q
-double bias_func(const Params& P, double thetae, int nsc) {
-  double b = P.bias0;
+// [parity unpinned] G21: b = max(1, bias0 * fac * Theta_e^p * (n_sc+1)^q), integer p, q; fac = the tuned factor of
+// generation n_sc (G32), 1 without tuning
+double bias_func(const Params& P, double thetae, int nsc, double fac) {
+  double b = P.bias0 * fac;
   for (int i = 0; i < P.bias_p_theta; i++) b *= thetae;
   for (int i = 0; i < P.bias_q_nsc; i++) b *= (double)(nsc + 1);
   return b > 1.0 ? b : 1.0;
@@ -105,7 +107,7 @@ void opacities(const Context& C, const double x[4], const double k[4], const Geo
   }
   if (P.scattering_on) {
     *nua_s = nu * S.ne * SIGMA_THOMSON * sigma_hot_eval(C.T, S.thetae, eps);
-    *bias = bias_func(P, S.thetae, nsc);
+    *bias = bias_func(P, S.thetae, nsc, C.bias_fac[nsc < 63 ? nsc : 63]);
   }
 }
 
@@ -153,7 +155,8 @@ static void fill_trace(TraceRec* tr, const Photon& p, int fate, double Einf, int
   tr->ith = ith; tr->inu = inu; tr->jscat = p.jscat; tr->pad_ = 0;
 }
 
-static void track_one(const Context& C, Photon p, std::vector<Photon>* stack, Tally* tl, Stats* st, TraceRec* tr) {
+static void track_one(const Context& C, Photon p, std::vector<Photon>* stack, Tally* tl, Stats* st, TraceRec* tr,
+                      int64_t* gen_spawn) {
   const Params& P = C.P;
   const double Cfac = HPL * P.L_unit / (ME * CL * CL);
   for (;;) {
@@ -235,6 +238,7 @@ static void track_one(const Context& C, Photon p, std::vector<Photon>* stack, Ta
             double kc[4]; lower(Ge.gcov, c.k, kc); c.E0 = -kc[0];
             stack->push_back(c);
             st->n_spawned++; st->sum_w_spawned += wc;
+            if (gen_spawn) gen_spawn[p.nsc < 63 ? p.nsc : 63]++;
           } else {
             st->n_bad_scatter++; st->sum_w_bad += wc;
           }
@@ -263,14 +267,14 @@ static void track_one(const Context& C, Photon p, std::vector<Photon>* stack, Ta
   }
 }
 
-void track_history(const Context& C, Photon ph, Tally* tl, Stats* st, TraceRec* root_trace) {
+void track_history(const Context& C, Photon ph, Tally* tl, Stats* st, TraceRec* root_trace, int64_t* gen_spawn) {
   std::vector<Photon> stack;
   st->n_primary++; st->sum_w_emit += ph.w; st->sum_wE_emit += ph.w * ph.E0;
-  track_one(C, ph, &stack, tl, st, root_trace);
+  track_one(C, ph, &stack, tl, st, root_trace, gen_spawn);
   while (!stack.empty()) {
     Photon c = stack.back();
     stack.pop_back();
-    track_one(C, c, &stack, tl, st, nullptr);
+    track_one(C, c, &stack, tl, st, nullptr, gen_spawn);
   }
 }
 
@@ -292,6 +296,7 @@ void run_range(Context* C, int64_t first, int64_t n, int nthreads) {
   if (nthreads < 1) nthreads = 1;
   std::vector<Tally> tls(nthreads);
   std::vector<Stats> sts(nthreads);
+  std::vector<std::vector<int64_t>> gens(nthreads, std::vector<int64_t>(64, 0));
   for (int t = 0; t < nthreads; t++) { tally_init(C->P, &tls[t]); sts[t] = Stats(); }
   const int64_t chunk = 1024;
   const int64_t nchunks = (n + chunk - 1) / chunk;
@@ -303,7 +308,7 @@ void run_range(Context* C, int64_t first, int64_t n, int nthreads) {
     for (int64_t pid = lo; pid < hi; pid++) {
       Photon ph;
       emit_photon(*C, pid, &ph);
-      track_history(*C, ph, &tls[t], &sts[t], nullptr);
+      track_history(*C, ph, &tls[t], &sts[t], nullptr, gens[t].data());
     }
   }
   size_t nb = C->tally.A.size();
@@ -313,7 +318,79 @@ void run_range(Context* C, int64_t first, int64_t n, int nthreads) {
       C->tally.W[b] += tls[t].W[b]; C->tally.n[b] += tls[t].n[b];
     }
     stats_add(&C->stats, sts[t]);
+    for (int g = 0; g < 64; g++) C->gen_spawn[g] += gens[t][g];
   }
+}
+
+// On-the-fly bias tuning (PAPER.md:369 names it as future work; the bias is there "to prevent
+// the number of generated superphotons from becoming excessive", 7-10x N_s in the GRMHD run).  Reading G32: the
+// separate scattered-superphoton generations give the counts for free, so one factor per generation is tuned on a
+// PILOT -- the first min(n, 32768) primaries and all their descendants, tracked into a scratch tally that is thrown
+// away -- until every generation with at least 200 parents spawns bias_target scattered superphotons per parent
+// within 5 % (|ln(ratio/target)| < 0.05).  Per generation and iteration, with r = spawned/parents:
+//   spawned < 50 (too few to steer by):  fac x 16; if the count has not grown three times running, the factor the
+//                                        climb started from is restored and the generation is frozen;
+//   else, closer to the target than ever: fac x clamp(target/r, 1/4, 4);
+//   else:                                 the best factor so far is restored and the generation is frozen.
+// (The ratio is not monotone in the bias: the gate w/b >= w_min removes children that a larger bias makes lighter, so
+// a generation can saturate below the target.)  A generation with fewer than 200 parents takes the factor of the one
+// before it.  At most 2 nsc_max + 8 iterations.  The factors are then frozen: the run proper does not depend on how it
+// is batched or sharded, and any bias leaves the spectrum unbiased
+// (test_scattered_spectrum_is_independent_of_the_bias).
+void tune_bias(Context* C, int nthreads) {
+  const Params& P = C->P;
+  std::fill(C->bias_fac.begin(), C->bias_fac.end(), 1.0);
+  C->tune_iterations = 0;
+  if (!P.bias_tune || !P.scattering_on || P.nsc_max < 1) return;
+  const int64_t n_all = C->offset.back();
+  const int64_t n_pilot = n_all < 32768 ? n_all : 32768;
+  if (n_pilot < 200) return;
+  const int G = P.nsc_max < 63 ? P.nsc_max : 63;           // generations 0 .. G-1 can scatter
+  Tally keep_t = C->tally; Stats keep_s = C->stats; std::vector<int64_t> keep_g = C->gen_spawn;
+  std::vector<double> best_fac(64, 1.0), best_err(64, 1e300), low_base(64, 1.0);
+  std::vector<int64_t> last_spawned(64, -1);
+  std::vector<int> low_fail(64, 0), in_low(64, 0);
+  std::vector<char> frozen(64, 0);
+  for (int iter = 0; iter < 2 * G + 8; iter++) {
+    tally_init(P, &C->tally); C->stats = Stats(); std::fill(C->gen_spawn.begin(), C->gen_spawn.end(), 0);
+    run_range(C, 0, n_pilot, nthreads);
+    C->tune_iterations = iter + 1;
+    bool done = true;
+    int64_t parents = n_pilot;
+    for (int g = 0; g < G; g++) {
+      const int64_t spawned = C->gen_spawn[g];
+      if (parents >= 200) {
+        if (!frozen[g]) {
+          const double r = (double)spawned / (double)parents;
+          const double err = spawned > 0 ? std::fabs(std::log(r / P.bias_target)) : 1e30;
+          if (!(err < 0.05)) {
+            done = false;
+            if (spawned < 50) {
+              if (!in_low[g]) { in_low[g] = 1; low_base[g] = C->bias_fac[g]; low_fail[g] = 0; last_spawned[g] = -1; }
+              low_fail[g] = spawned > last_spawned[g] ? 0 : low_fail[g] + 1;
+              last_spawned[g] = spawned;
+              if (low_fail[g] >= 3) { C->bias_fac[g] = low_base[g]; frozen[g] = 1; }
+              else C->bias_fac[g] *= 16.0;
+            } else if (err < best_err[g]) {
+              in_low[g] = 0;
+              best_err[g] = err; best_fac[g] = C->bias_fac[g];
+              double f = P.bias_target / r;
+              if (f > 4.0) f = 4.0;
+              if (f < 0.25) f = 0.25;
+              C->bias_fac[g] *= f;
+            } else {
+              C->bias_fac[g] = best_fac[g]; frozen[g] = 1;    // one more pass runs with the restored factor
+            }
+          }
+        }
+      } else if (g > 0 && !frozen[g]) {
+        C->bias_fac[g] = C->bias_fac[g - 1];
+      }
+      parents = spawned;
+    }
+    if (done) break;
+  }
+  C->tally = keep_t; C->stats = keep_s; C->gen_spawn = keep_g;
 }
 
 }  // namespace orc

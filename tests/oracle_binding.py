@@ -120,6 +120,8 @@ class OracleLib:
         L.orc_push.argtypes = [C.POINTER(Params)] + [C.c_void_p] * 3 + [C.c_double] + [C.c_void_p] * 3
         L.orc_geodesic.argtypes = [C.POINTER(Params), C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]
         L.orc_tetrad.argtypes = [C.POINTER(Params)] + [C.c_void_p] * 4
+        L.orc_get_bias_table.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        L.orc_set_bias_table.argtypes = [C.c_void_p, C.c_void_p]
         L.orc_zone_volume.restype = C.c_double
         L.orc_zone_volume.argtypes = [C.POINTER(Params), C.c_int, C.c_int, C.c_int]
         L.orc_sample_positions.argtypes = [C.POINTER(Params), C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p]
@@ -304,3 +306,14 @@ class Oracle:
         o = np.zeros(6)
         self.L.orc_fluid_frame(self.h, _p(x), _p(k), nsc, _p(o))
         return dict(eps=o[0], cos_b=o[1], nua_a=o[2], nua_s=o[3], bias=o[4], vacuum=bool(o[5]))
+
+    def bias_table(self):
+        """(per-generation bias factors [64], scattered superphotons spawned by each generation [64], pilot iterations)"""
+        f = np.zeros(64); g = np.zeros(64, dtype=np.int64)
+        it = self.L.orc_get_bias_table(self.h, _p(f), _p(g))
+        return f, g, it
+
+    def set_bias_table(self, fac):
+        f = np.ascontiguousarray(fac, dtype=np.float64)
+        assert f.size == 64
+        self.L.orc_set_bias_table(self.h, _p(f))
