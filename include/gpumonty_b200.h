@@ -171,6 +171,16 @@ int gm_set_batch(gm_ctx* ctx, int64_t batch_primaries, int64_t queue_records);
  * none.  k_cold >= 1.  Call before the first gm_run (run buffers are re-allocated). */
 int gm_set_phase_passes(gm_ctx* ctx, int pairs, int k_cold);
 
+/* Bias tuning (262-264, 304; G32).  With gm_params.bias_tune = 1, gm_prepare tunes one factor per
+ * scattering generation, b = max(1, bias0 fac[n_sc] Theta_e^p (n_sc+1)^q), on a pilot (the first min(n, 32768) primaries
+ * and their descendants, scratch tally) until each generation with >= 200 parents spawns gm_params.bias_target scattered
+ * superphotons per parent within 5 %; the factors are then frozen, so a run does not depend on its batching or sharding.
+ * gm_get_bias_table: fac[64] (may be NULL), gen_spawn[64] = scattered superphotons spawned by each generation since the
+ * last gm_reset_tally / gm_prepare (may be NULL), *pilot_passes (may be NULL).  gm_set_bias_table: install 64 factors
+ * (e.g. those another context tuned); gm_prepare resets them to 1 (or tunes them again). */
+int gm_get_bias_table(gm_ctx* ctx, double* fac, int64_t* gen_spawn, int* pilot_passes);
+int gm_set_bias_table(gm_ctx* ctx, const double* fac);
+
 /* nu L_nu [erg/s], its Monte Carlo sigma [erg/s] and the number of superphotons per [n_th][n_nu]
  * bin (O9).  Any of the three may be NULL. */
 int gm_get_spectrum(gm_ctx* ctx, double* nuLnu, double* sigma, int64_t* nphot);

@@ -24,7 +24,8 @@ FATE_ALIVE, FATE_RECORDED, FATE_HORIZON, FATE_ROULETTE, FATE_MAXSTEP, FATE_OUTOF
 
 EXPORTS = ["gm_create", "gm_destroy", "gm_last_error", "gm_set_grid", "gm_prepare", "gm_get_zone_counts",
            "gm_get_table", "gm_run", "gm_set_batch", "gm_set_phase_passes", "gm_get_spectrum", "gm_get_tally", "gm_get_stats",
-           "gm_reset_tally", "gm_emit", "gm_trace", "gm_eval", "gm_fp64_peak", "gm_build_tables", "gm_timing", "gm_spectrum_device"]
+           "gm_reset_tally", "gm_emit", "gm_trace", "gm_eval", "gm_fp64_peak", "gm_build_tables", "gm_timing", "gm_spectrum_device",
+           "gm_get_bias_table", "gm_set_bias_table"]
 
 
 class GmParams(C.Structure):
@@ -109,6 +110,8 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
     L.gm_build_tables.argtypes = [vp, vp]
     L.gm_spectrum_device.argtypes = [vp, vp, vp, vp]
     L.gm_timing.argtypes = [vp, C.c_int, vp, vp]
+    L.gm_get_bias_table.argtypes = [vp, vp, vp, C.POINTER(C.c_int)]
+    L.gm_set_bias_table.argtypes = [vp, vp]
     L.gm_abi_sizes.restype = None
     _lib = L
     return L
@@ -223,6 +226,17 @@ class GPUMonty:
         self._ck(self.L.gm_timing(self.h, int(enable), _np_ptr(ms), _np_ptr(nl)))
         names = ("tables", "prepare", "emit", "track", "compton", "spectrum", "escape")
         return {n: (float(ms[i]), int(nl[i])) for i, n in enumerate(names)}
+
+    def bias_table(self):
+        """(per-generation bias factors [64], scattered superphotons spawned by each generation [64], pilot passes)"""
+        f, g, it = np.zeros(64), np.zeros(64, dtype=np.int64), C.c_int(0)
+        self._ck(self.L.gm_get_bias_table(self.h, _np_ptr(f), _np_ptr(g), C.byref(it)))
+        return f, g, it.value
+
+    def set_bias_table(self, fac):
+        f = np.ascontiguousarray(fac, dtype=np.float64)
+        assert f.size == 64
+        self._ck(self.L.gm_set_bias_table(self.h, _np_ptr(f)))
 
     def reset_tally(self):
         self._ck(self.L.gm_reset_tally(self.h))

@@ -32,6 +32,7 @@ struct gm_ctx {
   int auto_pairs = -1;                             // the pilot's decision (-1: not taken yet)
   int carry_lanes = 4;                             // straggler hand-over threshold (0: off); GPUMONTY_B200_CARRY overrides
   double pilot_cold_fraction = -1.0;
+  int tune_iterations = 0;                         // bias tuning (G32): pilot passes of the last gm_prepare
   long long esc_records = 0;
   long long batch_primaries = 0, queue_records = 0;   // allocated sizes
   long long want_batch = 0, want_queue = 0;
@@ -161,6 +162,7 @@ static void fill_dev_params(gm_ctx* c) {
   P.max_steps = p.max_steps; P.verlet_maxit = p.verlet_maxit;
   P.scattering_on = p.scattering_on; P.nsc_max = p.nsc_max; P.bias_p = p.bias_p_theta; P.bias_q = p.bias_q_nsc;
   P.bias0 = p.bias0; P.roulette = p.roulette; P.inv_roulette = 1.0 / p.roulette;
+  for (int g = 0; g < 64; g++) P.bias_fac[g] = 1.0;
   P.n_th = p.n_th; P.n_nu = p.n_nu; P.fold_theta = p.fold_theta; P.emit_mode = p.emit_mode;
   P.nu_lo = p.nu_lo; P.db = std::log(p.nu_hi / p.nu_lo) / p.n_nu; P.inv_db = 1.0 / P.db;
   P.seed_lo = (uint32_t)(p.seed & 0xffffffffu); P.seed_hi = (uint32_t)(p.seed >> 32);
@@ -168,6 +170,8 @@ static void fill_dev_params(gm_ctx* c) {
 }
 
 extern "C" {
+
+static int tune_bias(gm_ctx* ctx, cudaStream_t st);
 
 const char* gm_last_error(const gm_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_err.c_str(); }
 
@@ -313,6 +317,8 @@ int gm_prepare(gm_ctx* ctx, void* cuda_stream, int64_t* n_primaries_out) {
   ctx->prepared = true;
   ctx->auto_pairs = -1;
   int r = gm_reset_tally(ctx);
+  if (r != GM_OK) return r;
+  r = tune_bias(ctx, st);                                   // G32: no-op unless bias_tune
   if (r != GM_OK) return r;
   if (n_primaries_out) *n_primaries_out = total;
   return GM_OK;
@@ -518,14 +524,9 @@ static int run_batch(gm_ctx* ctx, long long first, int n, const long long* d_ids
   return GM_OK;
 }
 
-int gm_run(gm_ctx* ctx, int64_t first_id, int64_t n_ids, void* cuda_stream) {
-  if (!ctx) return GM_ERR_PARAM;
-  if (!ctx->prepared) return fail(ctx, GM_ERR_STATE, "gm_run before gm_prepare");
-  if (first_id < 0 || n_ids < 0 || first_id + n_ids > ctx->n_primaries)
-    return fail(ctx, GM_ERR_PARAM, "id range [%lld,%lld) outside [0,%lld)", (long long)first_id,
-                (long long)(first_id + n_ids), ctx->n_primaries);
-  if (n_ids == 0) return GM_OK;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
+// Emit and transport the id range into `tally` / `stats` in batches; an overflowing batch is redone in smaller pieces
+// from a snapshot of the accumulators (nothing is dropped silently).
+static int run_range(gm_ctx* ctx, int64_t first_id, int64_t n_ids, Tally tally, DevStats* stats, cudaStream_t st) {
   int r = ensure_run_buffers(ctx, n_ids);
   if (r != GM_OK) return r;
   const int nb = ctx->p.n_th * ctx->p.n_nu;
@@ -536,14 +537,14 @@ int gm_run(gm_ctx* ctx, int64_t first_id, int64_t n_ids, void* cuda_stream) {
   while (done < n_ids) {
     long long nthis = n_ids - done < batch ? n_ids - done : batch;
     // snapshot so that an overflowing batch can be redone in smaller pieces (nothing is dropped silently)
-    CK(cudaMemcpyAsync(ctx->tally_snap.A, ctx->tally.A, (size_t)nb * 4 * sizeof(double), cudaMemcpyDeviceToDevice, st));
-    CK(cudaMemcpyAsync(ctx->d_stats_snap, ctx->d_stats, sizeof(DevStats), cudaMemcpyDeviceToDevice, st));
+    CK(cudaMemcpyAsync(ctx->tally_snap.A, tally.A, (size_t)nb * 4 * sizeof(double), cudaMemcpyDeviceToDevice, st));
+    CK(cudaMemcpyAsync(ctx->d_stats_snap, stats, sizeof(DevStats), cudaMemcpyDeviceToDevice, st));
     int mq = 0;
-    r = run_batch(ctx, first_id + done, (int)nthis, nullptr, notrace, false, ctx->tally, ctx->d_stats, st, &mq);
+    r = run_batch(ctx, first_id + done, (int)nthis, nullptr, notrace, false, tally, stats, st, &mq);
     if (r != GM_OK) return r;
     if (mq > ctx->queue_records) {
-      CK(cudaMemcpyAsync(ctx->tally.A, ctx->tally_snap.A, (size_t)nb * 4 * sizeof(double), cudaMemcpyDeviceToDevice, st));
-      CK(cudaMemcpyAsync(ctx->d_stats, ctx->d_stats_snap, sizeof(DevStats), cudaMemcpyDeviceToDevice, st));
+      CK(cudaMemcpyAsync(tally.A, ctx->tally_snap.A, (size_t)nb * 4 * sizeof(double), cudaMemcpyDeviceToDevice, st));
+      CK(cudaMemcpyAsync(stats, ctx->d_stats_snap, sizeof(DevStats), cudaMemcpyDeviceToDevice, st));
       if (nthis <= 256)
         return fail(ctx, GM_ERR_OVERFLOW, "scattered-superphoton queue (%lld records) overflows with a batch of %lld primaries; "
                     "raise it with gm_set_batch or lower the bias", ctx->queue_records, nthis);
@@ -555,6 +556,113 @@ int gm_run(gm_ctx* ctx, int64_t first_id, int64_t n_ids, void* cuda_stream) {
     }
     done += nthis;
   }
+  return GM_OK;
+}
+
+int gm_run(gm_ctx* ctx, int64_t first_id, int64_t n_ids, void* cuda_stream) {
+  if (!ctx) return GM_ERR_PARAM;
+  if (!ctx->prepared) return fail(ctx, GM_ERR_STATE, "gm_run before gm_prepare");
+  if (first_id < 0 || n_ids < 0 || first_id + n_ids > ctx->n_primaries)
+    return fail(ctx, GM_ERR_PARAM, "id range [%lld,%lld) outside [0,%lld)", (long long)first_id,
+                (long long)(first_id + n_ids), ctx->n_primaries);
+  if (n_ids == 0) return GM_OK;
+  return run_range(ctx, first_id, n_ids, ctx->tally, ctx->d_stats, (cudaStream_t)cuda_stream);
+}
+
+// On-the-fly bias tuning (262-264, 304; G32): one factor per scattering generation, tuned on a
+// pilot -- the first min(n, 32768) primaries and their descendants, tracked into a scratch tally -- until every
+// generation with >= 200 parents spawns bias_target scattered superphotons per parent within 5 %; the rule is stated
+// in DESIGN.md G32 (low counts: x16 until the count stops growing; otherwise x clamp(target/ratio, 1/4, 4) while the
+// generation gets closer to the target, else back to its best factor and frozen).  One read-back of the 64
+// per-generation counters per pilot pass.  The factors are frozen afterwards.
+static int tune_bias(gm_ctx* ctx, cudaStream_t st) {
+  const gm_params& p = ctx->p;
+  for (int g = 0; g < 64; g++) ctx->P.bias_fac[g] = 1.0;
+  ctx->tune_iterations = 0;
+  if (!p.bias_tune || !p.scattering_on || p.nsc_max < 1) return GM_OK;
+  const long long n_pilot = ctx->n_primaries < 32768 ? ctx->n_primaries : 32768;
+  if (n_pilot < 200) return GM_OK;
+  const int G = p.nsc_max < 63 ? p.nsc_max : 63;
+  const int nb = p.n_th * p.n_nu;
+  double* d_tl = nullptr; DevStats* d_st = nullptr;
+  CK(cudaMalloc((void**)&d_tl, (size_t)nb * 4 * sizeof(double)));
+  if (cudaMalloc((void**)&d_st, sizeof(DevStats)) != cudaSuccess) { cudaFree(d_tl); return fail(ctx, GM_ERR_CUDA, "tune_bias: allocation failed"); }
+  Tally scratch{d_tl, d_tl + nb, d_tl + 2 * nb, (unsigned long long*)(d_tl + 3 * nb)};
+  double best_fac[64], best_err[64], low_base[64];
+  long long last_spawned[64];
+  int low_fail[64], in_low[64], frozen[64];
+  for (int g = 0; g < 64; g++) { best_fac[g] = 1.0; best_err[g] = 1e300; low_base[g] = 1.0; last_spawned[g] = -1; low_fail[g] = in_low[g] = frozen[g] = 0; }
+  int rc = GM_OK;
+  DevStats* h = new DevStats;
+  for (int iter = 0; iter < 2 * G + 8 && rc == GM_OK; iter++) {
+    cudaMemsetAsync(d_tl, 0, (size_t)nb * 4 * sizeof(double), st);
+    cudaMemsetAsync(d_st, 0, sizeof(DevStats), st);
+    rc = run_range(ctx, 0, n_pilot, scratch, d_st, st);
+    if (rc != GM_OK) break;
+    if (cudaMemcpyAsync(h, d_st, sizeof(DevStats), cudaMemcpyDeviceToHost, st) != cudaSuccess || cudaStreamSynchronize(st) != cudaSuccess) {
+      rc = fail(ctx, GM_ERR_CUDA, "tune_bias: read-back failed"); break;
+    }
+    ctx->tune_iterations = iter + 1;
+    bool done = true;
+    long long parents = n_pilot;
+    for (int g = 0; g < G; g++) {
+      const long long spawned = (long long)h->gen[g];
+      double& fac = ctx->P.bias_fac[g];
+      if (parents >= 200) {
+        if (!frozen[g]) {
+          const double r = (double)spawned / (double)parents;
+          const double err = spawned > 0 ? std::fabs(std::log(r / p.bias_target)) : 1e30;
+          if (!(err < 0.05)) {
+            done = false;
+            if (spawned < 50) {
+              if (!in_low[g]) { in_low[g] = 1; low_base[g] = fac; low_fail[g] = 0; last_spawned[g] = -1; }
+              low_fail[g] = spawned > last_spawned[g] ? 0 : low_fail[g] + 1;
+              last_spawned[g] = spawned;
+              if (low_fail[g] >= 3) { fac = low_base[g]; frozen[g] = 1; }
+              else fac *= 16.0;
+            } else if (err < best_err[g]) {
+              in_low[g] = 0;
+              best_err[g] = err; best_fac[g] = fac;
+              double f = p.bias_target / r;
+              f = f > 4.0 ? 4.0 : (f < 0.25 ? 0.25 : f);
+              fac *= f;
+            } else {
+              fac = best_fac[g]; frozen[g] = 1;
+            }
+          }
+        }
+      } else if (g > 0 && !frozen[g]) {
+        fac = ctx->P.bias_fac[g - 1];
+      }
+      parents = spawned;
+    }
+    if (done) break;
+  }
+  delete h;
+  cudaFree(d_tl); cudaFree(d_st);
+  return rc;
+}
+
+int gm_get_bias_table(gm_ctx* ctx, double* fac, int64_t* gen_spawn, int* pilot_passes) {
+  if (!ctx) return GM_ERR_PARAM;
+  if (fac) for (int g = 0; g < 64; g++) fac[g] = ctx->P.bias_fac[g];
+  if (gen_spawn) {
+    DevStats* h = new DevStats;
+    cudaError_t e = cudaDeviceSynchronize();
+    if (e == cudaSuccess) e = cudaMemcpy(h, ctx->d_stats, sizeof(DevStats), cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess) for (int g = 0; g < 64; g++) gen_spawn[g] = (int64_t)h->gen[g];
+    delete h;
+    if (e != cudaSuccess) return fail(ctx, GM_ERR_CUDA, "gm_get_bias_table: %s", cudaGetErrorString(e));
+  }
+  if (pilot_passes) *pilot_passes = ctx->tune_iterations;
+  return GM_OK;
+}
+
+int gm_set_bias_table(gm_ctx* ctx, const double* fac) {
+  if (!ctx || !fac) return GM_ERR_PARAM;
+  for (int g = 0; g < 64; g++)
+    if (!(fac[g] > 0.0) || !std::isfinite(fac[g])) return fail(ctx, GM_ERR_PARAM, "bias factor %d must be positive and finite", g);
+  for (int g = 0; g < 64; g++) ctx->P.bias_fac[g] = fac[g];
   return GM_OK;
 }
 

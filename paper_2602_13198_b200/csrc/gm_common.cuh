@@ -54,6 +54,7 @@ struct DevParams {
   // scattering
   int scattering_on, nsc_max, bias_p, bias_q, pad1;
   double bias0, roulette, inv_roulette;
+  double bias_fac[64];                                // tuned factor per scattering generation (G32); 1 without tuning
   // tally
   int n_th, n_nu, fold_theta, emit_mode;
   double nu_lo, inv_db, db;
@@ -80,6 +81,7 @@ static_assert(sizeof(Photon) == 160, "Photon record must be 160 bytes");
 struct DevStats {
   unsigned long long n[15];
   double s[12];
+  unsigned long long gen[64];                         // scattered superphotons spawned by generation n_sc (G32)
 };
 enum { SN_PRIMARY = 0, SN_SPAWNED, SN_RECORDED, SN_HORIZON, SN_ROUL_KILLED, SN_ROUL_SURV, SN_MAXSTEP,
        SN_OUTOFRANGE, SN_STEPS, SN_VITERS, SN_VCAPPED, SN_BADSCAT, SN_ANALOG, SN_STEPS_FREE, SN_REENTER };

@@ -907,6 +907,11 @@ __global__ void __launch_bounds__(128, GM_COMPTON_MINBLOCKS) compton_kernel(cons
       ph.nsc += 1; ph.nstep = 0; ph.jscat = 0; ph.flags = 0;
       opacities(P, ph.k, G, S, ph.nsc, P.scattering_on != 0 && ph.nsc < P.nsc_max, ph.nua_a, ph.nua_s, ph.bias);
       c_spawn++; s_spawn += ph.w;
+      {                                                    // per-generation count (bias tuning, G32): one atomic per warp and generation
+        const int g = ph.nsc - 1;
+        const unsigned peers = __match_any_sync(__activemask(), g);
+        if ((int)(threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(&stats->gen[g & 63], (unsigned long long)__popc(peers));
+      }
       if (trace.rec && ph.root >= 0) atomicAdd((unsigned long long*)&trace.rec[ph.root].fam_nspawn, 1ull);
     } else {
       ph.flags = FLAG_DEAD;

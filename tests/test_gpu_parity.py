@@ -639,6 +639,41 @@ def test_contexts_on_disjoint_id_ranges_sum_to_the_single_run(gm, cfg, world):
             assert st_acc[k] == pytest.approx(v, rel=1e-11, abs=1e-300), k
 
 
+@pytest.mark.parametrize("cfg", ["sphere", "torus"])
+def test_bias_tuning_matches_the_oracle_and_meets_its_target(gm, cfg):
+    """bias_tune = 1 (G32): gm_prepare tunes one bias factor per scattering
+    generation on a pilot.  Same integer counts on both sides => the same factors, bit for bit; the run proper then
+    matches the oracle history by history, and every generation with enough parents spawns the target number of
+    scattered superphotons per parent.  A context given the oracle's table explicitly (no pilot) gives the same run."""
+    if cfg == "sphere":
+        p, prim = wl.config1(Ns=1e5, seed=3, nu_min=1e10, nu_max=1e13, bias0=1.0, bias_q_nsc=0, nsc_max=3,
+                             bias_tune=1, bias_target=0.5, w_min=0.0)
+        target, gens = 0.5, 3
+    else:
+        p, prim = wl.config2(Ns=3e4, bias0=1.0, bias_tune=1, bias_target=2.19)
+        target, gens = 2.19, 2
+    o, g = _pair(gm, p, prim)
+    fo, _, ito = o.bias_table()
+    fg, _, itg = g.bias_table()
+    assert itg == ito and np.array_equal(fo, fg), (ito, itg, fo[:4], fg[:4])
+    o.run(); g.run()
+    _compare_stats(o, g, rel=5e-3)
+    _, gen_o, _ = o.bias_table()
+    _, gen_g, _ = g.bias_table()
+    assert np.array_equal(gen_o, gen_g)
+    parents = g.n_primaries
+    for k in range(gens):
+        assert abs(gen_g[k] / parents / target - 1) < 0.15, (k, gen_g[k], parents)
+        parents = gen_g[k]
+    _compare_traces(o, g, np.arange(0, g.n_primaries, 13), fork_budget=2e-4)
+    q = dict(p); q["bias_tune"] = 0
+    g2 = gm.GPUMonty(q); g2.set_grid(prim); g2.prepare(); g2.set_bias_table(fo); g2.run()
+    assert np.array_equal(g2.tally()[3], g.tally()[3])
+    if cfg == "torus":
+        sg = g.stats()
+        assert sg["n_spawned"] / sg["n_primary"] == pytest.approx(7.0, abs=0.7)      # PAPER.md:304, no calibrated bias0
+
+
 def test_small_first_request_does_not_pin_the_batch_size(gm):
     """a small gm_trace / gm_run used to fix the internal batch at its own size, so that a later
     full-size gm_run was cut into thousands of tiny batches.  The buffers are re-sized now: the large run after a
