@@ -37,15 +37,17 @@ METRIC = "superphotons/s tracked (incl. scattering)"
 UNIT = "superphotons/s"
 # algorithmic FP64 flop per geodesic step (dadd + dmul + 2 dfma predicated-on thread
 # instructions of the kernel divided by the steps it committed, counted with ncu on each workload class with the
-# single mixed tracker pass, so that no redone step is counted -- profiles/r01f_final.md -- and then
-# frozen).  "track": in-grid step of track_kernel; "escape": free-flight step of escape_kernel.
-FLOP_PER_STEP = {"flat": {"track": 717.6, "escape": 208.0}, "kerr": {"track": 704.7, "escape": 368.2},
-                 "kerr3d": {"track": 807.5, "escape": 368.2}}
+# single mixed tracker pass, so that no redone step is counted -- profiles/r02_final.md, r02j_flops_cfg*.csv -- and
+# then frozen).  "track": in-grid step of track_kernel; "escape": free-flight step of escape_kernel.
+FLOP_PER_STEP = {"flat": {"track": 705.8, "escape": 208.0}, "kerr": {"track": 693.7, "escape": 368.2},
+                 "kerr3d": {"track": 808.5, "escape": 368.2}}
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant launch from one ncu --set full capture; a constant of
 # that capture (its command and N_s are named in TRAFFIC_SOURCE), not a quantity measured in this run.  The run
 # itself reports the ALGORITHMIC bytes per launch beside it (roofline.algorithmic_bytes_per_launch).
-TRAFFIC_BYTES_PER_LAUNCH = {2: 85.4e6 + 76.2e6}
-TRAFFIC_SOURCE = {2: "profiles/r01g_carry_over.md: cold tracker pass over 1.09e6 primaries, cfg2 at N_s=3e6 (NOT this run's N_s)"}
+TRAFFIC_BYTES_PER_LAUNCH = {2: 274.7e6 + 364.2e6}
+TRAFFIC_SOURCE = {2: "profiles/r02_final.md (ncu --set full of this workload, cfg2 at N_s=1e7): first cold tracker pass, "
+                     "11.8 ms under ncu; reads the 1.7e6 records the hot pass parked, writes 2.3e6 hand-over / free-flight / "
+                     "scattered records of 160 B: DRAM traffic = algorithmic record bytes, the gather is served by L1/L2"}
 WORKLOAD_NAMES = {0: "cfg0 thin synchrotron sphere 32x16, Ns=1e5", 1: "cfg1 scattering sphere 32x16, Ns=1e6",
                   2: "cfg2 Kerr FM torus 256x256, Ns=1e7", 3: "cfg3 3-D perturbed torus 192x128x128, Ns=1e7",
                   4: "cfg4 Kerr torus x1e3 density (analog scattering), Ns=1e6"}

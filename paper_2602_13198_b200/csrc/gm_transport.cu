@@ -648,69 +648,44 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
 // A superphoton that comes back below x1hi (possible only for grids that end inside the photon orbit) is
 // appended to `ret` as a complete record and tracked by the next tracker launch.
 template <bool KERR>
-#ifndef GM_ESC_BATCH
-#define GM_ESC_BATCH 32
-#endif
 #ifndef GM_ESC_MINBLOCKS
 #define GM_ESC_MINBLOCKS 4
 #endif
 __global__ void __launch_bounds__(128, GM_ESC_MINBLOCKS)
 escape_kernel(const __grid_constant__ DevParams P, Queue esc, int* work_counter, Queue ret, Tally tally, DevStats* stats,
               TraceBuf trace, int* overflow) {
-  // persistent, refilled like the tracker: the 32 lanes of a warp step together, stopped lanes take the next
-  // records from a shared-memory stage that is loaded 32 records at a time (coalesced, ahead of their use)
-  __shared__ uint4 s_stage[4][32 * PH_U4];
+  // Persistent; the 32 lanes of a warp step together and are refilled together (see below): each lane reads its own
+  // record of the next 32-record chunk straight from the queue.  Chunks are handed out by an atomic counter (flight
+  // lengths differ: a warp waits for its slowest lane, so static assignment ran 17 % slower), but the counter is read
+  // one refill AHEAD: the atomic for the chunk after next is issued when a chunk is taken, and its result is not
+  // touched until the following refill, a whole flight later.  (Round 2: with all warps of a launch refilling at about
+  // the same moments, the counter's round trip was 16 % of this kernel's stall samples, profiles/r02_tracker_study.md.)
   const int n = min(*esc.count, esc.capacity);
   if (blockIdx.x == 0 && threadIdx.x == 0 && *esc.count > esc.capacity) atomicOr(overflow, 2);
-  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  const unsigned lt_mask = (1u << lane) - 1u;
-  uint4* stage = s_stage[wid];
-  unsigned c_steps = 0, c_viters = 0;             // per thread and launch: far below 2^32
+  const int lane = threadIdx.x & 31;
+  int next_base = 0;                                // lane 0: first record of the chunk this warp takes next
+  if (lane == 0) next_base = atomicAdd(work_counter, 32);
+  unsigned c_steps = 0, c_viters = 0;               // per thread and launch: far below 2^32
   Lane L;
   L.w = 0.0; L.nua_a = 0.0; L.nua_s = 0.0; L.bias = 1.0;
   L.id0 = L.id1 = L.id2 = L.nstep = L.jscat = 0u; L.nsc = 0; L.root = -1; L.flags = 0;
 #pragma unroll
   for (int m = 0; m < 4; m++) { L.x[m] = 0.0; L.k[m] = 0.0; L.a[m] = 0.0; }
-  bool have = false, exhausted = false, arrived = false;
-  int st_next = 0, st_avail = 0;
+  bool have = false, arrived = false;
   for (;;) {
     __syncwarp();
-    unsigned need = __ballot_sync(0xffffffffu, !have);
+    const unsigned need = __ballot_sync(0xffffffffu, !have);
     // Every history of this kernel ends at r_max, and recording one lane at a time was 44 % of its samples (lane
     // copy in local memory, generic atomics, 1.3 live lanes; profiles/r01f).  So the lanes that arrived wait until
-    // GM_ESC_BATCH lanes of the warp need a refill; then they record together -- inline, with reductions -- and are
-    // refilled together.  Free flights from the grid edge to r_max have nearly equal lengths, so even waiting for
-    // the whole warp (32) idles little: measured 74.8 / 65.0 / 62.8 / 61.4 / 60.3 ms for 1 / 4 / 8 / 16 / 32.
-    if (__popc(need) < GM_ESC_BATCH && !exhausted) need = 0;
-    if (need) {
+    // the whole warp needs a refill; then they record together -- inline, with reductions -- and are refilled
+    // together: measured 74.8 / 65.0 / 62.8 / 61.4 / 60.3 ms for groups of 1 / 4 / 8 / 16 / 32.
+    if (need == 0xffffffffu) {
       if (arrived) { record_core<KERR, true>(P, L, tally, stats, trace); arrived = false; }
-      __syncwarp();
-      if (st_next == st_avail && !exhausted) {
-        int base = 0;
-        if (lane == 0) base = atomicAdd(work_counter, 32);
-        base = __shfl_sync(0xffffffffu, base, 0);
-        const int cnt = min(32, n - base);
-        if (cnt <= 0) {
-          exhausted = true;
-        } else {
-          const uint4* src = reinterpret_cast<const uint4*>(esc.buf + base);
-          for (int i = lane; i < cnt * PH_U4; i += 32) stage[i] = __ldg(src + i);
-          st_next = 0; st_avail = cnt;
-        }
-        __syncwarp();
-      }
-      const int left = st_avail - st_next;
-      if (left > 0) {
-        const int rank = __popc(need & lt_mask);
-        if (!have && rank < left) {
-          lane_load(L, reinterpret_cast<const Photon*>(stage) + st_next + rank);
-          have = true;
-        }
-        st_next += min(__popc(need), left);
-        __syncwarp();
-      } else if (exhausted && need == 0xffffffffu) {
-        break;
-      }
+      const int base = __shfl_sync(0xffffffffu, next_base, 0);
+      const int cnt = min(32, n - base);
+      if (cnt <= 0) break;                                   // queue used up
+      if (lane == 0) next_base = atomicAdd(work_counter, 32);   // for the refill after this one
+      if (lane < cnt) { lane_load(L, esc.buf + base + lane); have = true; }
     }
     if (!have) continue;
     if (L.flags & FLAG_CARRY) {                            // a tracker straggler: on to the next generation, as it is
