@@ -254,7 +254,7 @@ def _compare_traces(o, g, ids, fork_budget, label=None):
     """Same-stream histories one by one.  A history "forks" when a uniform falls within rounding of a threshold
     (or libdevice and glibc differ in the last ulp of a transcendental): every integer of its final state is
     compared, the forks are counted, printed and (on the GPU box) appended to gpurun_out/fork_rates.md; the budget
-    is a bound on that measured rate (<= 3x what profiles/r02_fork_rates.md records)."""
+    is a bound on that measured rate (<= 3x what profiles/r02_parity.md records)."""
     tg = g.trace(ids)
     to, fam_wE, fam_n = o.trace(ids)
     same = (tg["fate"] == to["fate"]) & (tg["nstep"] == to["nstep"]) & (tg["inu"] == to["inu"]) & \
