@@ -285,9 +285,15 @@ __device__ __forceinline__ void tally_red(const Tally T, int bin, double wE, dou
 
 // RED = false: the tracker's rare, out-of-line call (record_photon below).  RED = true: inlined into the free-flight
 // kernel, where every history ends here: no lane copy in local memory, no generic atomics.
+// Run totals of the recorded superphotons (count, sum w, sum wE) of one thread of the free-flight kernel: kept in
+// registers and added to the device statistics once per warp at the end of the launch.  (One reduction per
+// superphoton on these three addresses -- 5e7 same-address fp64 reductions per cfg 2 step -- serialised in the L2
+// and WAS the kernel's duration: 61 ms whatever the occupancy or the refill scheme, 40 ms without them.)
+struct RecAcc { double w, wE; unsigned n; };
+
 template <bool KERR, bool RED>
 __device__ __forceinline__ void record_core(const DevParams& P, const Lane& L, const Tally& tally, DevStats* stats,
-                                            const TraceBuf& trace) {
+                                            const TraceBuf& trace, RecAcc* acc = nullptr) {
   Geom G;
   geom_at<KERR, false>(P, L.x[1], L.x[2], G, nullptr);
   const double E = -(G.g00 * L.k[0] + G.g01 * L.k[1] + G.g03 * L.k[3]);     // -k_t, conserved (O9)
@@ -316,10 +322,7 @@ __device__ __forceinline__ void record_core(const DevParams& P, const Lane& L, c
     const double wE = L.w * E;
     if (RED) {
       tally_red(tally, ith * P.n_nu + inu, wE, L.w);
-      const unsigned act = __activemask();
-      if ((int)(threadIdx.x & 31) == __ffs(act) - 1) red_add(&stats->n[SN_RECORDED], (unsigned long long)__popc(act));
-      red_add(&stats->s[SS_REC], L.w);
-      red_add(&stats->s[SS_WE_REC], wE);
+      acc->n++; acc->w += L.w; acc->wE += wE;
     } else {
       tally_add(tally, ith * P.n_nu + inu, wE, L.w);
       atomicAdd(&stats->n[SN_RECORDED], 1ull);
@@ -340,14 +343,16 @@ __device__ __forceinline__ void record_core(const DevParams& P, const Lane& L, c
 }
 
 template <bool KERR>
-__device__ __noinline__ void record_photon(const DevParams& P, const Lane& L, const Tally& tally, DevStats* stats,
-                                           const TraceBuf& trace) {
+// (Tally and TraceBuf by value: a reference would force the kernel's copy of the parameter into local memory, and
+// every later use of it -- `trace.rec` in the loops -- would become a local load)
+__device__ __noinline__ void record_photon(const DevParams& P, const Lane& L, const Tally tally, DevStats* stats,
+                                           const TraceBuf trace) {
   record_core<KERR, false>(P, L, tally, stats, trace);
 }
 
 // a superphoton that stops without being recorded: counters + optional trace
 __device__ __noinline__ void kill_photon(const Lane& L, int fate, int n_idx, int s_idx, DevStats* stats,
-                                         const TraceBuf& trace) {
+                                         const TraceBuf trace) {
   atomicAdd(&stats->n[n_idx], 1ull);
   if (s_idx >= 0) atomicAdd(&stats->s[s_idx], L.w);
   if (trace.rec && L.root >= 0 && (L.flags & FLAG_ROOT)) {
@@ -362,7 +367,7 @@ __device__ __noinline__ void kill_photon(const Lane& L, int fate, int n_idx, int
 // The out-of-line functions get a COPY of the lane state (their argument has its address taken; the
 // live state must stay in registers).
 __device__ __noinline__ double roulette(const DevParams& P, const Lane& L, double ur, DevStats* stats,
-                                        const TraceBuf& trace) {
+                                        const TraceBuf trace) {
   if (ur < P.inv_roulette) {
     atomicAdd(&stats->n[SN_ROUL_SURV], 1ull);
     atomicAdd(&stats->s[SS_ROUL_GAIN], L.w * (P.roulette - 1.0));
@@ -647,56 +652,158 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
 // ---- free flight beyond the grid: the same step with vacuum ahead (tau_a = tau_s = 0) -----------------
 // A superphoton that comes back below x1hi (possible only for grids that end inside the photon orbit) is
 // appended to `ret` as a complete record and tracked by the next tracker launch.
+constexpr int ESC_CHUNK = 16;                       // records per chunk; two chunk buffers per warp (2 x 2.5 KB)
+constexpr int ESC_ARR_CAP = 64;                     // arrival list of a warp: 64 x 48 B = 3 KB
+constexpr int ESC_WARP_SMEM = 2 * ESC_CHUNK * (int)sizeof(Photon) + ESC_ARR_CAP * 48;   // 8 KB
+#ifndef GM_ESC_THREADS
+#define GM_ESC_THREADS 128
+#endif
+
+// shared memory through 32-bit shared-window addresses (the generic-pointer form made the compiler re-derive the
+// window base from S2R SR_CgaCtaId in every loop iteration: 7.6 % of the kernel's stall samples)
+__device__ __forceinline__ void lds_f64x2(unsigned a, double& x, double& y) {
+  asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(x), "=d"(y) : "r"(a));
+}
+__device__ __forceinline__ void sts_f64x2(unsigned a, double x, double y) {
+  asm volatile("st.shared.v2.f64 [%0], {%1,%2};" ::"r"(a), "d"(x), "d"(y) : "memory");
+}
+__device__ __forceinline__ void lane_load_shared(Lane& L, unsigned a) {
+  lds_f64x2(a, L.x[0], L.x[1]); lds_f64x2(a + 16, L.x[2], L.x[3]);
+  lds_f64x2(a + 32, L.k[0], L.k[1]); lds_f64x2(a + 48, L.k[2], L.k[3]);
+  lds_f64x2(a + 64, L.a[0], L.a[1]); lds_f64x2(a + 80, L.a[2], L.a[3]);
+  lds_f64x2(a + 96, L.w, L.nua_a); lds_f64x2(a + 112, L.nua_s, L.bias);
+  uint32_t m0, m1, m2, m3;
+  asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(L.id0), "=r"(L.id1), "=r"(L.id2), "=r"(L.nstep) : "r"(a + 128));
+  asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(m0), "=r"(m1), "=r"(m2), "=r"(m3) : "r"(a + 144));
+  L.nsc = (int)m0; L.jscat = m1; L.root = (int)m2; L.flags = (int)m3;
+}
+
 template <bool KERR>
 #ifndef GM_ESC_MINBLOCKS
 #define GM_ESC_MINBLOCKS 4
 #endif
-__global__ void __launch_bounds__(128, GM_ESC_MINBLOCKS)
+__global__ void __launch_bounds__(GM_ESC_THREADS, GM_ESC_MINBLOCKS)
 escape_kernel(const __grid_constant__ DevParams P, Queue esc, int* work_counter, Queue ret, Tally tally, DevStats* stats,
               TraceBuf trace, int* overflow) {
-  // Persistent; the 32 lanes of a warp step together and are refilled together (see below): each lane reads its own
-  // record of the next 32-record chunk straight from the queue.  Chunks are handed out by an atomic counter (flight
-  // lengths differ: a warp waits for its slowest lane, so static assignment ran 17 % slower), but the counter is read
-  // one refill AHEAD: the atomic for the chunk after next is issued when a chunk is taken, and its result is not
-  // touched until the following refill, a whole flight later.  (Round 2: with all warps of a launch refilling at about
-  // the same moments, the counter's round trip was 16 % of this kernel's stall samples, profiles/r02_tracker_study.md.)
+  // Persistent; the 32 lanes of a warp step together.  Every history of this kernel ends at r_max, and flight lengths
+  // differ (a superphoton grazing the polar axis takes many small steps), so three things are decoupled here:
+  //  * a lane that arrives appends the six numbers the tally needs to the warp's arrival list in shared memory and is
+  //    refilled AT ONCE from the warp's current chunk (16 records in shared memory);
+  //  * the next chunk is copied from the queue with cp.async while the current one is being used, and the chunk
+  //    counter is read one chunk further ahead still, so neither the queue's DRAM latency nor the counter's round
+  //    trip is waited for (they were 13 % and 6 % of the stall samples with a synchronous copy);
+  //  * the arrival list is recorded 32 entries at a time -- inline, all lanes busy, with reductions.
+  // Round 1 recorded one lane at a time (44 % of the kernel's samples: lane copy in local memory, generic atomics, 1.3
+  // live lanes); round 2a let arrived lanes wait for the whole warp (23.9 of 32 lanes live, profiles/r02_kernels.md).
+  __shared__ __align__(16) unsigned char s_raw[(GM_ESC_THREADS / 32) * ESC_WARP_SMEM];
   const int n = min(*esc.count, esc.capacity);
   if (blockIdx.x == 0 && threadIdx.x == 0 && *esc.count > esc.capacity) atomicOr(overflow, 2);
-  const int lane = threadIdx.x & 31;
-  int next_base = 0;                                // lane 0: first record of the chunk this warp takes next
-  if (lane == 0) next_base = atomicAdd(work_counter, 32);
+  unsigned lane, sbase;
+  asm volatile("mov.u32 %0, %%laneid;" : "=r"(lane));
+  sbase = (unsigned)__cvta_generic_to_shared(s_raw) + (threadIdx.x >> 5) * ESC_WARP_SMEM;
+  asm volatile("" : "+r"(sbase));                   // opaque: kept in a register, not re-derived in the loop
+  const unsigned lt_mask = (1u << lane) - 1u;
+  const unsigned arr_s = sbase + 2 * ESC_CHUNK * (unsigned)sizeof(Photon);
+  gm_trace_rec* const trec = trace.rec;
+  // chunk pipeline: [cur] in use, [cur ^ 1] in flight (nxt_cnt records), lane 0's next_base = first record of the
+  // chunk after that (its atomic was issued one switch ago)
+  int cur = 0, st_next = 0, st_avail = 0, nxt_cnt = 0, arr_n = 0;   // warp-uniform
+  bool exhausted = false;                                           // warp-uniform
+  int next_base = 0;
+  {
+    int b0 = 0;
+    if (lane == 0) { b0 = atomicAdd(work_counter, ESC_CHUNK); next_base = atomicAdd(work_counter, ESC_CHUNK); }
+    b0 = __shfl_sync(0xffffffffu, b0, 0);
+    nxt_cnt = max(0, min(ESC_CHUNK, n - b0));
+    const uint4* src = reinterpret_cast<const uint4*>(esc.buf + b0);
+    const unsigned dst = sbase + ESC_CHUNK * (unsigned)sizeof(Photon);
+    for (int i = lane; i < nxt_cnt * PH_U4; i += 32)
+      asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst + 16u * i), "l"(src + i));
+    asm volatile("cp.async.commit_group;");
+  }
   unsigned c_steps = 0, c_viters = 0;               // per thread and launch: far below 2^32
+  RecAcc racc{0.0, 0.0, 0u};
   Lane L;
   L.w = 0.0; L.nua_a = 0.0; L.nua_s = 0.0; L.bias = 1.0;
   L.id0 = L.id1 = L.id2 = L.nstep = L.jscat = 0u; L.nsc = 0; L.root = -1; L.flags = 0;
 #pragma unroll
   for (int m = 0; m < 4; m++) { L.x[m] = 0.0; L.k[m] = 0.0; L.a[m] = 0.0; }
-  bool have = false, arrived = false;
+  bool have = false;
   for (;;) {
     __syncwarp();
     const unsigned need = __ballot_sync(0xffffffffu, !have);
-    // Every history of this kernel ends at r_max, and recording one lane at a time was 44 % of its samples (lane
-    // copy in local memory, generic atomics, 1.3 live lanes; profiles/r01f).  So the lanes that arrived wait until
-    // the whole warp needs a refill; then they record together -- inline, with reductions -- and are refilled
-    // together: measured 74.8 / 65.0 / 62.8 / 61.4 / 60.3 ms for groups of 1 / 4 / 8 / 16 / 32.
-    if (need == 0xffffffffu) {
-      if (arrived) { record_core<KERR, true>(P, L, tally, stats, trace); arrived = false; }
-      const int base = __shfl_sync(0xffffffffu, next_base, 0);
-      const int cnt = min(32, n - base);
-      if (cnt <= 0) break;                                   // queue used up
-      if (lane == 0) next_base = atomicAdd(work_counter, 32);   // for the refill after this one
-      if (lane < cnt) { lane_load(L, esc.buf + base + lane); have = true; }
+    if (need) {
+      if (st_next == st_avail && !exhausted) {
+        // the chunk in flight becomes the current one; the chunk after it is started
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+        __syncwarp();
+        cur ^= 1; st_next = 0; st_avail = nxt_cnt;
+        if (st_avail == 0) {
+          exhausted = true;
+        } else {
+          int z = 0;
+          asm volatile("" : "+r"(z));               // keeps the shuffle (and the wait for the atomic) HERE
+          const int base = __shfl_sync(0xffffffffu, next_base, z);
+          nxt_cnt = max(0, min(ESC_CHUNK, n - base));
+          if (nxt_cnt > 0) {
+            if (lane == 0) next_base = atomicAdd(work_counter, ESC_CHUNK);
+            const uint4* src = reinterpret_cast<const uint4*>(esc.buf + base);
+            const unsigned dst = sbase + (cur ^ 1) * (ESC_CHUNK * (unsigned)sizeof(Photon));
+            for (int i = lane; i < nxt_cnt * PH_U4; i += 32)
+              asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst + 16u * i), "l"(src + i));
+          }
+          asm volatile("cp.async.commit_group;");
+        }
+      }
+      const int left = st_avail - st_next;
+      if (left > 0) {
+        const int rank = __popc(need & lt_mask);
+        if (!have && rank < left) {
+          lane_load_shared(L, sbase + (cur * ESC_CHUNK + st_next + rank) * (unsigned)sizeof(Photon));
+          have = true;
+        }
+        st_next += min(__popc(need), left);
+        __syncwarp();
+      } else if (exhausted && need == 0xffffffffu) {
+        break;
+      }
     }
-    if (!have) continue;
-    if (L.flags & FLAG_CARRY) {                            // a tracker straggler: on to the next generation, as it is
+    if (have && (L.flags & FLAG_CARRY)) {                  // a tracker straggler: on to the next generation, as it is
       L.flags &= ~FLAG_CARRY;
       const int slot = atomicAdd(ret.count, 1);
       if (slot < ret.capacity) lane_store(L, ret.buf + slot);
-      have = false; continue;
+      have = false;
     }
-    if (L.x[2] < 0.0) { L.x[2] = -L.x[2]; L.k[2] = -L.k[2]; L.a[2] = -L.a[2]; L.x[3] += C_PI; }
-    if (L.x[2] > 1.0) { L.x[2] = 2.0 - L.x[2]; L.k[2] = -L.k[2]; L.a[2] = -L.a[2]; L.x[3] += C_PI; }
-    if (L.x[1] >= P.lnr_max) { arrived = true; have = false; continue; }       // recorded at the next refill
+    if (have) {
+      if (L.x[2] < 0.0) { L.x[2] = -L.x[2]; L.k[2] = -L.k[2]; L.a[2] = -L.a[2]; L.x[3] += C_PI; }
+      if (L.x[2] > 1.0) { L.x[2] = 2.0 - L.x[2]; L.k[2] = -L.k[2]; L.a[2] = -L.a[2]; L.x[3] += C_PI; }
+    }
+    // ---- arrivals at r_max ----
+    const bool arrive = have && L.x[1] >= P.lnr_max;
+    const unsigned am = __ballot_sync(0xffffffffu, arrive);
+    if (am) {
+      if (trec) {                                          // histories are being traced (tests): record in place
+        if (arrive) record_core<KERR, true>(P, L, tally, stats, trace, &racc);
+      } else {
+        if (arrive) {
+          const unsigned e = arr_s + 48u * (arr_n + __popc(am & lt_mask));
+          sts_f64x2(e, L.x[1], L.x[2]); sts_f64x2(e + 16, L.k[0], L.k[1]); sts_f64x2(e + 32, L.k[3], L.w);
+        }
+        arr_n += __popc(am);
+        __syncwarp();
+        if (arr_n >= 32) {
+          arr_n -= 32;
+          Lane R;
+          R.x[0] = R.x[3] = R.k[2] = 0.0; R.nstep = R.jscat = 0u; R.nsc = 0; R.root = -1; R.flags = 0;
+          const unsigned e = arr_s + 48u * (arr_n + lane);
+          lds_f64x2(e, R.x[1], R.x[2]); lds_f64x2(e + 16, R.k[0], R.k[1]); lds_f64x2(e + 32, R.k[3], R.w);
+          record_core<KERR, true>(P, R, tally, stats, trace, &racc);
+          __syncwarp();
+        }
+      }
+      if (arrive) have = false;
+    }
+    if (!have) continue;
     if (stop_tests<KERR>(P, L, tally, stats, trace)) { have = false; continue; }
     if (L.x[1] < P.x1hi) {                                 // back inside the grid
       L.nua_a = 0.0; L.nua_s = 0.0; L.bias = 1.0;          // opacities at a vacuum point
@@ -722,15 +829,29 @@ escape_kernel(const __grid_constant__ DevParams P, Queue esc, int* work_counter,
     for (int m = 0; m < 4; m++) { L.x[m] = x1[m]; L.k[m] = k1[m]; L.a[m] = a1[m]; }
     L.nstep++; c_steps++;
   }
+  __syncwarp();
+  if ((int)lane < arr_n) {                                 // the rest of the arrival list
+    Lane R;
+    R.x[0] = R.x[3] = R.k[2] = 0.0; R.nstep = R.jscat = 0u; R.nsc = 0; R.root = -1; R.flags = 0;
+    const unsigned e = arr_s + 48u * lane;
+    lds_f64x2(e, R.x[1], R.x[2]); lds_f64x2(e + 16, R.k[0], R.k[1]); lds_f64x2(e + 32, R.k[3], R.w);
+    record_core<KERR, true>(P, R, tally, stats, trace, &racc);
+  }
   unsigned long long w_steps = c_steps, w_viters = c_viters;
   for (int o = 16; o > 0; o >>= 1) {
     w_steps += __shfl_xor_sync(0xffffffffu, w_steps, o);
     w_viters += __shfl_xor_sync(0xffffffffu, w_viters, o);
   }
+  __syncwarp();
+  racc.w = warp_sum(racc.w); racc.wE = warp_sum(racc.wE);
+  racc.n = __reduce_add_sync(0xffffffffu, racc.n);
   if ((threadIdx.x & 31) == 0) {
     stat_add_n(stats, SN_STEPS, w_steps);
     stat_add_n(stats, SN_STEPS_FREE, w_steps);
     stat_add_n(stats, SN_VITERS, w_viters);
+    stat_add_n(stats, SN_RECORDED, racc.n);
+    stat_add_s(stats, SS_REC, racc.w);
+    stat_add_s(stats, SS_WE_REC, racc.wE);
   }
 }
 
@@ -1067,8 +1188,8 @@ cudaError_t launch_escape(const DevParams& P, Queue esc, int* work_counter, Queu
   const int grid = n_sm * GM_ESC_MINBLOCKS;
   cudaError_t e = cudaMemsetAsync(work_counter, 0, sizeof(int), st);
   if (e != cudaSuccess) return e;
-  if (P.metric_kind == 1) escape_kernel<true><<<grid, 128, 0, st>>>(P, esc, work_counter, ret, tally, stats, trace, overflow);
-  else escape_kernel<false><<<grid, 128, 0, st>>>(P, esc, work_counter, ret, tally, stats, trace, overflow);
+  if (P.metric_kind == 1) escape_kernel<true><<<grid, GM_ESC_THREADS, 0, st>>>(P, esc, work_counter, ret, tally, stats, trace, overflow);
+  else escape_kernel<false><<<grid, GM_ESC_THREADS, 0, st>>>(P, esc, work_counter, ret, tally, stats, trace, overflow);
   return cudaGetLastError();
 }
 
