@@ -17,22 +17,25 @@
 namespace gm {
 
 // ------------------------------------------------------------------------------------------------
+// one warp per node: the lanes share the terms of the sum (a single thread per node left each of these two
+// kernels a 224-term dependent chain on 201 / 261 threads: 0.07 + 0.24 ms of every gm_build_tables)
 __global__ void k2_table_kernel(double* __restrict__ lnK2) {
-  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   if (i > NK2) return;
   const double l0 = log(K2_TMIN), dl = log(K2_TMAX / K2_TMIN) / NK2;
   double x = 1.0 / exp(l0 + i * dl);
   // trapezoid in t with step 1/16; the integrand falls below 1e-300 before t = 14 for x >= 0.01
   const double h = 1.0 / 16.0;
-  double sum = 0.5 * exp(-x);
-  for (int n = 1; n < 16 * 14; n++) {
+  double sum = lane == 0 ? 0.5 * exp(-x) : 0.0;
+  for (int n = 1 + lane; n < 16 * 14; n += 32) {
     double t = n * h;
     double ch = cosh(t);
     double arg = x * ch;
     if (arg > 745.0) break;
     sum += exp(-arg) * cosh(2.0 * t);
   }
-  lnK2[i] = log(sum * h);
+  sum = warp_sum(sum);
+  if (lane == 0) lnK2[i] = log(sum * h);
 }
 
 __device__ __forceinline__ double F_integrand(double K, double s) {
@@ -43,7 +46,7 @@ __device__ __forceinline__ double F_integrand(double K, double s) {
   return s * s * t * t * exp(-x13);
 }
 __global__ void f_table_kernel(double* __restrict__ lnF) {
-  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
   if (i > NF) return;
   const double k0 = log(F_KMIN), dk = log(F_KMAX / F_KMIN) / NF;
   double K = exp(k0 + i * dk);
@@ -52,7 +55,7 @@ __global__ void f_table_kernel(double* __restrict__ lnF) {
   const double h = 1.0 / 32.0;
   const int N = 112;   // t in [-3.5, 3.5]
   double sum = 0.0;
-  for (int n = -N; n <= N; n++) {
+  for (int n = -N + lane; n <= N; n += 32) {
     double t = n * h;
     double u = 0.5 * C_PI * sinh(t);
     double e2 = exp(-2.0 * fabs(u));
@@ -61,7 +64,8 @@ __global__ void f_table_kernel(double* __restrict__ lnF) {
     double s = (u < 0.0) ? sin(delta) : cos(delta);        // theta = delta or pi/2 - delta
     sum += wgt * F_integrand(K, s);
   }
-  lnF[i] = log(4.0 * C_PI * sum * h);
+  sum = warp_sum(sum);
+  if (lane == 0) lnF[i] = log(4.0 * C_PI * sum * h);
 }
 
 // Gauss-Legendre nodes/weights on [-1,1]
@@ -139,11 +143,11 @@ __global__ void __launch_bounds__(128) sigh_table_kernel(double* __restrict__ ln
 }
 
 cudaError_t build_K2_table(double* d, cudaStream_t st) {
-  k2_table_kernel<<<(NK2 + 128) / 128, 128, 0, st>>>(d);
+  k2_table_kernel<<<(NK2 + 4) / 4, 128, 0, st>>>(d);
   return cudaGetLastError();
 }
 cudaError_t build_F_table(double* d, cudaStream_t st) {
-  f_table_kernel<<<(NF + 64) / 64, 64, 0, st>>>(d);
+  f_table_kernel<<<(NF + 4) / 4, 128, 0, st>>>(d);
   return cudaGetLastError();
 }
 cudaError_t build_sigh_table(double* d, cudaStream_t st) {
