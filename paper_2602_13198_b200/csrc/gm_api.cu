@@ -19,6 +19,7 @@ struct gm_ctx {
   long nz = 0;
   // device memory
   double* d_prim = nullptr;
+  double2* d_cellB = nullptr;                     // per-cell bounds of the cold pass (nz entries)
   double *d_lnK2 = nullptr, *d_lnF = nullptr, *d_lnSigH = nullptr, *d_lnw = nullptr;
   ZoneArrays Z{};
   int n_weight_blocks = 0;
@@ -92,7 +93,7 @@ static void free_run_buffers(gm_ctx* c) {
 static void free_all(gm_ctx* c) {
   if (!c) return;
   free_run_buffers(c);
-  cudaFree(c->d_prim); cudaFree(c->d_lnK2); cudaFree(c->d_lnF); cudaFree(c->d_lnSigH); cudaFree(c->d_lnw);
+  cudaFree(c->d_prim); cudaFree(c->d_cellB); cudaFree(c->d_lnK2); cudaFree(c->d_lnF); cudaFree(c->d_lnSigH); cudaFree(c->d_lnw);
   cudaFree(c->Z.A); cudaFree(c->Z.nu0); cudaFree(c->Z.vol); cudaFree(c->Z.Nexp); cudaFree(c->Z.qmax);
   cudaFree(c->Z.n); cudaFree(c->Z.offset); cudaFree(c->Z.partial); cudaFree(c->Z.nu_nodes); cudaFree(c->Z.wk);
   cudaFree(c->Z.blocksum); cudaFree(c->Z.bad);
@@ -166,6 +167,7 @@ static void fill_dev_params(gm_ctx* c) {
   P.n_th = p.n_th; P.n_nu = p.n_nu; P.fold_theta = p.fold_theta; P.emit_mode = p.emit_mode;
   P.nu_lo = p.nu_lo; P.db = std::log(p.nu_hi / p.nu_lo) / p.n_nu; P.inv_db = 1.0 / P.db;
   P.seed_lo = (uint32_t)(p.seed & 0xffffffffu); P.seed_hi = (uint32_t)(p.seed >> 32);
+  P.cellB = c->d_cellB;
   P.prim = c->d_prim; P.lnK2 = c->d_lnK2; P.lnF = c->d_lnF; P.lnSigH = c->d_lnSigH; P.lnw = c->d_lnw;
 }
 
@@ -206,6 +208,7 @@ int gm_create(gm_ctx** out, const gm_params* p) {
   auto A = [&](void** ptr, size_t bytes) { return cudaMalloc(ptr, bytes ? bytes : 8); };
   bool ok = true;
   ok = ok && A((void**)&ctx->d_prim, nz * 8 * sizeof(double)) == cudaSuccess;
+  ok = ok && A((void**)&ctx->d_cellB, nz * sizeof(double2)) == cudaSuccess;
   ok = ok && A((void**)&ctx->d_lnK2, (NK2 + 1) * sizeof(double)) == cudaSuccess;
   ok = ok && A((void**)&ctx->d_lnF, (NF + 1) * sizeof(double)) == cudaSuccess;
   ok = ok && A((void**)&ctx->d_lnSigH, (size_t)(NSE + 1) * (NST + 1) * sizeof(double)) == cudaSuccess;
@@ -367,7 +370,7 @@ static int phase_pairs_of(const gm_ctx* ctx) {
   if (ctx->p.metric_kind != 1) return 0;                 // instantiated for the Kerr workloads only
   if (ctx->phase_pairs >= 0) return ctx->phase_pairs;
   if (ctx->p.thetae_mode == 0) return 0;                 // a uniform Theta_e has no cold phase
-  return ctx->auto_pairs >= 0 ? ctx->auto_pairs : 2;
+  return ctx->auto_pairs >= 0 ? ctx->auto_pairs : 3;
 }
 
 int gm_set_phase_passes(gm_ctx* ctx, int pairs, int k_cold) {
@@ -487,7 +490,7 @@ static int run_batch(gm_ctx* ctx, long long first, int n, const long long* d_ids
             CK(cudaMemcpyAsync(&parked, parkA.count, sizeof(int), cudaMemcpyDeviceToHost, st));
             CK(cudaStreamSynchronize(st));
             ctx->pilot_cold_fraction = (double)parked / (double)n;
-            ctx->auto_pairs = ctx->pilot_cold_fraction >= 0.35 ? 2 : 0;
+            ctx->auto_pairs = ctx->pilot_cold_fraction >= 0.35 ? 3 : 0;
             if (getenv("GPUMONTY_B200_DEBUG"))
               fprintf(stderr, "[gpumonty_b200] %.3f of the primaries leave the first hot pass alive -> %d pass pairs\n",
                       ctx->pilot_cold_fraction, ctx->auto_pairs);

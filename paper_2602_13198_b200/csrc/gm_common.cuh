@@ -66,6 +66,9 @@ struct DevParams {
   const double* __restrict__ lnF;
   const double* __restrict__ lnSigH;
   const double* __restrict__ lnw;
+  // per interpolation cell (indexed like its lowest corner zone): {S, Theta_B}, upper bounds of the scattering
+  // opacity per unit k^t and of Theta_e anywhere in the cell (cell_bound_kernel; the tracker's cold pass)
+  const double2* __restrict__ cellB;
 };
 
 // ---- superphoton record (160 B, 16-B aligned) -------------------------------------------------

@@ -330,8 +330,74 @@ __global__ void __launch_bounds__(256) scan_tile_kernel(const int32_t* __restric
   for (int i = 0; i < 4; i++) { long z = base + i; if (z < nz) offset[z] = run; run += v[i]; }
 }
 
+// ------------------------------------------------------------------------------------------------
+// Upper bounds per interpolation cell, for the tracker's cold pass (DESIGN.md section 6 "bounded steps").
+// The plasma state at a point is derived from the multilinear interpolant of the primitives between the 4 (2-D)
+// or 8 (3-D) zone centres around it (G4): a convex combination.  Over such a cell
+//   n_e = rho Ne_unit                       <= max_c rho_c Ne_unit;
+//   u/rho of the interpolant                <= max_c u_c/rho_c (mediant inequality), hence
+//   Theta_e (G3)                            <= its value at that ratio, in mode 2 with the smallest R the cell allows:
+//                                            R rises with beta^2 = N^2/D^2 (for R_high >= R_low), N = (gam-1) u >=
+//                                            (gam-1) min_c u_c, D = b^2/2 <= g_ij B^i B^j / 2 (b^2 <= alpha^2 g_ij B^i B^j,
+//                                            the normal observer's field), convex in B^i; capped by thetae_max;
+//   gamma^2 = 1 + g_ij u~^i u~^j (convex in u~) <= 1 + 100 max_c q_c, q_c formed with the metric at corner c: the
+//                                            factor covers the variation of g_ij over the cell and the half zones
+//                                            beyond the outermost centres (sin^2 theta changes by <= 9 next to the axis);
+//   eps = -k.u = gamma E_n (1 - v.n)        <= gamma (1 + v) E_n,  E_n = alpha k^t <= k^t (alpha = (1+f)^-1/2 <= 1),
+//                                            gamma (1 + v) = gamma + sqrt(gamma^2 - 1), rising with gamma;
+//   sigma_h / sigma_T                       <= 1.
+// So nu alpha_s <= k^t S with S = (gamma_B + sqrt(gamma_B^2 - 1)) n_e,B sigma_T m_e c^2/h, and the bias b(Theta_e) <= b(Theta_B) (G21 is
+// non-decreasing in Theta_e).  Each bound carries a margin of 1e-6 against the rounding of the exact evaluation.
+// A cell whose state cannot be bounded (non-finite input, u > 0 on rho = 0) gets Theta_B = inf: never skipped.
+template <bool KERR>
+__global__ void cell_bound_kernel(const DevParams P, double2* __restrict__ cellB, long nz) {
+  long z = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (z >= nz) return;
+  const int k3 = (int)(z % P.n3), j2 = (int)((z / P.n3) % P.n2), i1 = (int)(z / ((long)P.n3 * P.n2));
+  double rho_max = 0.0, ratio_max = 0.0, q_max = 0.0, bb_max = 0.0, u_min = INFINITY;
+  bool ok = true;
+  for (int di = 0; di < 2; di++)
+    for (int dj = 0; dj < 2; dj++)
+      for (int dk = 0; dk < 2; dk++) {
+        const int i = min(i1 + di, P.n1 - 1), j = min(j2 + dj, P.n2 - 1);
+        const int k = P.n3 > 1 ? (k3 + dk) % P.n3 : 0;
+        double pr[8];
+        load_zone(P.prim, ((long)i * P.n2 + j) * P.n3 + k, pr);
+#pragma unroll
+        for (int q = 0; q < 8; q++) ok = ok && isfinite(pr[q]);
+        Geom G;
+        geom_at<KERR, false>(P, P.startx1 + (i + 0.5) * P.dx1, P.startx2 + (j + 0.5) * P.dx2, G, nullptr);
+        const double q = G.g11 * pr[2] * pr[2] + 2.0 * fabs(G.g13 * pr[2] * pr[4]) + G.g22 * pr[3] * pr[3] + G.g33 * pr[4] * pr[4];
+        q_max = fmax(q_max, q);
+        bb_max = fmax(bb_max, G.g11 * pr[5] * pr[5] + 2.0 * fabs(G.g13 * pr[5] * pr[7]) + G.g22 * pr[6] * pr[6] + G.g33 * pr[7] * pr[7]);
+        u_min = fmin(u_min, pr[1]);
+        rho_max = fmax(rho_max, pr[0]);
+        if (pr[0] > 0.0) ratio_max = fmax(ratio_max, pr[1] / pr[0]);
+        else if (pr[1] > 0.0 || pr[0] < 0.0) ok = false;
+      }
+  double thB;
+  if (P.thetae_mode == 0) thB = P.thetae_fixed;
+  else if (P.thetae_mode == 1) thB = (C_MP / C_ME) * (P.gam_ad - 1.0) * ratio_max / (1.0 + P.trat);
+  else {
+    double Rmin = fmin(P.R_low, P.R_high);
+    if (P.R_high >= P.R_low && u_min > 0.0) {
+      const double N = (P.gam_ad - 1.0) * u_min, D = 0.5 * 100.0 * bb_max;
+      const double N2 = N * N, D2 = D * D;
+      if (isfinite(N2) && isfinite(D2) && N2 + D2 > 0.0) Rmin = (P.R_high * N2 + P.R_low * D2) / (N2 + D2) * (1.0 - 1e-6);
+    }
+    thB = (C_MP / C_ME) * (2.0 / 3.0) * ratio_max / (2.0 + Rmin);
+  }
+  thB = fmin(thB * (1.0 + 1e-6), P.thetae_max);
+  const double gamB = sqrt(1.0 + 100.0 * q_max);
+  double S = (gamB + sqrt(100.0 * q_max)) * (rho_max * P.Ne_unit) * C_SIGT * C_MEC2_H * (1.0 + 1e-6);
+  if (!ok || !isfinite(S) || !isfinite(thB)) { S = INFINITY; thB = INFINITY; }
+  cellB[z] = make_double2(S, thB);
+}
+
 cudaError_t launch_prepare(const DevParams& P, const ZoneArrays& Z, double* d_lnw, long nz, cudaStream_t st) {
   int nb128 = (int)((nz + 127) / 128);
+  if (P.metric_kind == 1) cell_bound_kernel<true><<<nb128, 128, 0, st>>>(P, const_cast<double2*>(P.cellB), nz);
+  else cell_bound_kernel<false><<<nb128, 128, 0, st>>>(P, const_cast<double2*>(P.cellB), nz);
   if (P.metric_kind == 1) zone_state_kernel<true><<<nb128, 128, 0, st>>>(P, Z, nz);
   else zone_state_kernel<false><<<nb128, 128, 0, st>>>(P, Z, nz);
   int nblk = (int)((nz + 255) / 256);

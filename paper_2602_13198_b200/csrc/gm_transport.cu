@@ -18,6 +18,7 @@ namespace gm {
 constexpr int FLAG_ROOT = 1, FLAG_DEAD = 2;
 constexpr int FLAG_ROULETTED = 4;   // the roulette of step `nstep` was already played (record moved between passes)
 constexpr int FLAG_CARRY = 8;       // straggler handed to the next generation's launch through the free-flight queue
+constexpr int FLAG_BOUND = 16;      // nua_s and bias of the record are upper bounds, not the values at x (cold pass, see track_kernel)
 
 // ---- block-level stats helper ---------------------------------------------------------------------
 __device__ __forceinline__ void stat_add_n(DevStats* st, int which, unsigned long long v) {
@@ -204,6 +205,9 @@ __global__ void __launch_bounds__(128, GM_EMIT_MINBLOCKS) emit_kernel(const DevP
 // A history is a pure function of its record (counter-based RNG), so the passes change no result.
 // =====================================================================================================
 constexpr int PHASE_MIXED = 0, PHASE_HOT = 1, PHASE_COLD = 2;
+#ifndef GM_QUIET_BT
+#define GM_QUIET_BT (1.0 / 64.0)
+#endif
 #ifndef GM_TRACK_THREADS
 #define GM_TRACK_THREADS 128
 #endif
@@ -394,6 +398,35 @@ __device__ __forceinline__ bool stop_tests(const DevParams& P, Lane& L, const Ta
   return false;
 }
 
+// ---- bounded steps of the cold pass ---------------------------------------------
+// A step needs the plasma state at its end point for two things: the scattering test (b tau_s against the uniform
+// u of this step) and the absorption.  Far from the torus both are decided without it: the cell's
+// Theta_B < thetae_min rules out absorption, and with the cell's bounds (cell_bound_kernel) b_B tau_s,B <= u rules
+// out the event, because x_r = -ln(1-u) >= u and every factor of b tau_s is below its bound.  The cold pass takes
+// only such steps -- no gather, no plasma state, no opacity: the free-flight step plus one 16-byte load -- and
+// commits them with the BOUNDS stored in (nua_s, bias) and FLAG_BOUND set.  A superphoton whose next step is not
+// decided this way (possibly hot plasma, b_B tau_s,B > u, or a reflection at the axis with bounds in the record)
+// is handed to the next hot pass with its start-of-step state.  There a FLAG_BOUND record first takes a step of
+// length zero (mode 3): the ordinary gather / plasma / opacity code, all lanes of the warp busy with their own steps,
+// forms the exact (nua_s, bias) at the record's point; then it continues as usual.  Every decision is the one the
+// exact evaluation takes, so no history changes (the parity tests compare them one by one).
+template <bool THREED>
+__device__ __forceinline__ long cell_index(const DevParams& P, const double x[4]) {
+  int i0, i1, j0, j1;
+  double w;
+  axis_weights(x[1], P.startx1, P.inv_dx1, P.n1, i0, i1, w);
+  double x2 = x[2];
+  if (x2 < 0.0) x2 = -x2;
+  if (x2 > 1.0) x2 = 2.0 - x2;
+  axis_weights(x2, P.startx2, P.inv_dx2, P.n2, j0, j1, w);
+  long z = ((long)i0 * P.n2 + j0) * P.n3;
+  if (THREED) {
+    const long kk = (long)floor((x[3] - P.startx3) * P.inv_dx3 - 0.5), n3 = P.n3;
+    z += ((kk % n3) + n3) % n3;
+  }
+  return z;
+}
+
 #ifndef GM_TRACK_MINBLOCKS
 #define GM_TRACK_MINBLOCKS 3
 #endif
@@ -432,7 +465,6 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
   int ncold = 0;                        // PHASE_HOT: consecutive committed cold steps of this lane
   int mode = 0;                         // 0 normal step, 1 partial push to a scattering event, 2 redo full step
   double dl = 0.0, ux = 0.0, ev_f = 0.0, ev_b = 1.0, ev_tau = 0.0;
-  int ev_it = 0;                        // PHASE_COLD: Verlet iterations counted for the attempt that found the event
   int st_next = 0, st_avail = 0;        // staged records [st_next, st_avail); warp-uniform
   bool exhausted = false;               // warp-uniform
   unsigned c_steps = 0, c_viters = 0;            // per thread and launch: far below 2^32
@@ -491,6 +523,19 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
     }
     if (!have) continue;
 
+    if (PHASE == PHASE_COLD) mode = 0;                     // (the cold pass has no events: lets the compiler drop their code)
+    if (mode == 0) {
+      if (L.flags & FLAG_BOUND) {
+        if (PHASE != PHASE_COLD) {
+          mode = 3; dl = 0.0;                               // step of length zero: exact opacities at the record's point
+        } else if (L.x[2] < 0.0 || L.x[2] > 1.0) {
+          // the reflection below changes the point the exact values belong to (G33): the hot pass forms them first
+          const int slot = atomicAdd(park.count, 1);
+          if (slot < park.capacity) lane_store(L, park.buf + slot);
+          have = false; continue;
+        }
+      }
+    }
     if (mode == 0) {
       if (stop_tests<KERR>(P, L, tally, stats, trace)) { have = false; continue; }
       if (L.x[1] >= P.x1hi && L.k[1] > 0.0) {              // leaves the grid outwards: free flight
@@ -522,6 +567,31 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
     double pr[8];
     bool inplasma = false;
     int it;
+    Plasma S;
+    double na1 = 0.0, ns1 = 0.0, b1 = 1.0;
+    bool hot = false;
+    bool bnd1 = false;                                     // (ns1, b1) are the cell's bounds
+    bool quiet = true;                                     // PHASE_HOT: b tau_s of this step far below 1
+    if (PHASE == PHASE_COLD) {
+      const bool ingrid = x1[1] >= P.x1lo && x1[1] < P.x1hi;
+      double2 cb = make_double2(0.0, 0.0);
+      if (ingrid) cb = __ldg(P.cellB + cell_index<THREED>(P, x1));      // flies during the push
+      it = push_wavevector<KERR>(P, L.k, L.a, dl_eff, x1, k1, a1, G, capped);
+      bool decided = !ingrid;                              // beyond the grid: vacuum, (0, 1) exactly
+      if (ingrid && cb.y < P.thetae_min && k1[0] > 0.0) {  // certainly not hot: the cell's bounds stand in
+        decided = true; bnd1 = true;
+        if (want_scat) { ns1 = k1[0] * cb.x; b1 = bias_func(P, cb.y, L.nsc); }
+      }
+      // b tau_s <= its bound <= u <= x_r: no event.  Otherwise (or if the plasma may be hot) the step is not taken here.
+      if (decided && want_scat && 0.5 * (L.bias + b1) * (0.5 * (L.nua_s + ns1) * P.Cfac * dl) > ux) decided = false;
+      if (L.nua_a != 0.0) decided = false;                 // (a start point in hot plasma: absorption is the hot pass's)
+      if (!decided) {
+        const int slot = atomicAdd(park.count, 1);
+        if (slot < park.capacity) lane_store(L, park.buf + slot);
+        have = false;
+        continue;
+      }
+    } else
     if (STAGED) {
       GatherW gw;
       const bool ingrid = gather_issue<THREED>(P, x1, sg, gw);     // asynchronous copies fly during the push
@@ -531,30 +601,18 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
       inplasma = interp_prim<THREED>(P, x1, pr) && pr[0] > 0.0;
       it = push_wavevector<KERR>(P, L.k, L.a, dl_eff, x1, k1, a1, G, capped);
     }
-    Plasma S;
-    double na1 = 0.0, ns1 = 0.0, b1 = 1.0;
-    bool hot = false;
-    if (inplasma) {
+    if (PHASE != PHASE_COLD && inplasma) {
       plasma_from_prim(P, G, pr, S);
       hot = S.thetae >= P.thetae_min && S.B > 0.0;         // the condition under which opacities() absorbs
-      if (PHASE == PHASE_COLD) {
-        if (hot) {                                         // park the start-of-step state for the next hot pass
-          const int slot = atomicAdd(park.count, 1);
-          if (slot < park.capacity) lane_store(L, park.buf + slot);
-          if (mode != 0) {                                 // the attempt of this step is redone: uncount it
-            c_viters -= (unsigned)abs(ev_it);
-            if (ev_it < 0) atomicAdd(&stats->n[SN_VCAPPED], ~0ull);
-          }
-          have = false; mode = 0;
-          continue;
-        }
-        opacities<false>(P, k1, G, S, L.nsc, want_scat, na1, ns1, b1);
-      } else {
-        opacities<true>(P, k1, G, S, L.nsc, want_scat, na1, ns1, b1);
-      }
+      opacities<true>(P, k1, G, S, L.nsc, want_scat, na1, ns1, b1);
     }
 
-    if (mode == 1) {
+    if (PHASE != PHASE_COLD && mode == 3) {                // zero-length step of a FLAG_BOUND record: its exact opacities
+      L.nua_s = ns1; L.bias = b1; L.flags &= ~FLAG_BOUND;
+      mode = 0;
+      continue;
+    }
+    if (PHASE != PHASE_COLD && mode == 1) {
       // ---- scattering event at x1 ----
       if (!(inplasma && S.ne > 0.0)) { mode = 2; continue; }   // event point in vacuum: full step instead (G30)
       c_viters += it; if (capped) atomicAdd(&stats->n[SN_VCAPPED], 1ull);
@@ -579,7 +637,7 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
       L.jscat++;
       L.nua_a = na1; L.nua_s = ns1; L.bias = b1;
       L.nstep++; c_steps++;
-      L.flags &= ~FLAG_ROULETTED;
+      L.flags &= ~(FLAG_ROULETTED | FLAG_BOUND);             // (an event point is always evaluated exactly)
       mode = 0;
       if (!(L.w > 0.0)) {                                    // analog limit b = 1
         const Lane T = L;
@@ -589,12 +647,13 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
       continue;
     }
 
-    const double tau_a = 0.5 * (L.nua_a + na1) * P.Cfac * dl;          // Eq. 20
+    const double tau_a = PHASE == PHASE_COLD ? 0.0 : 0.5 * (L.nua_a + na1) * P.Cfac * dl;          // Eq. 20
     if (mode == 0) {
       c_viters += it; if (capped) atomicAdd(&stats->n[SN_VCAPPED], 1ull);
-      if (want_scat) {
+      if (PHASE != PHASE_COLD && want_scat) {              // (the cold pass commits only steps decided above)
         const double tau_s = 0.5 * (L.nua_s + ns1) * P.Cfac * dl;      // Eq. 25
         const double bt = 0.5 * (L.bias + b1) * tau_s;                 // G19
+        quiet = bt < GM_QUIET_BT;
         // x_r = -ln(1-u) >= u: the logarithm is needed only when b tau_s exceeds u
         const double b = 0.5 * (L.bias + b1);
         // w/b >= w_min is the other condition of the event (G21): a weight below half of w_min b cannot meet it,
@@ -603,7 +662,6 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
           const double xr = -log(1.0 - ux);
           if (bt > xr && L.w / b >= P.w_min) {
             mode = 1; ev_f = xr / bt; ev_b = b; ev_tau = tau_a;
-            if (PHASE == PHASE_COLD) ev_it = capped ? -it : it;
             continue;
           }
         }
@@ -619,10 +677,10 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
     for (int m = 0; m < 4; m++) { L.x[m] = x1[m]; L.k[m] = k1[m]; L.a[m] = a1[m]; }
     L.nua_a = na1; L.nua_s = ns1; L.bias = b1;
     L.nstep++; c_steps++;
-    L.flags &= ~FLAG_ROULETTED;
+    L.flags = (L.flags & ~(FLAG_ROULETTED | FLAG_BOUND)) | (bnd1 ? FLAG_BOUND : 0);
     mode = 0;
     if (PHASE == PHASE_HOT) {
-      ncold = hot ? 0 : ncold + 1;
+      ncold = (hot || !quiet) ? 0 : ncold + 1;             // quiet: a step the cold pass could have decided with its bounds
       if (ncold >= k_cold && L.x[1] < P.x1hi) {            // cold for k_cold steps: continue in the cold pass
         const int slot = atomicAdd(park.count, 1);
         if (slot < park.capacity) lane_store(L, park.buf + slot);
@@ -807,6 +865,7 @@ escape_kernel(const __grid_constant__ DevParams P, Queue esc, int* work_counter,
     if (stop_tests<KERR>(P, L, tally, stats, trace)) { have = false; continue; }
     if (L.x[1] < P.x1hi) {                                 // back inside the grid
       L.nua_a = 0.0; L.nua_s = 0.0; L.bias = 1.0;          // opacities at a vacuum point
+      L.flags &= ~FLAG_BOUND;
       const int slot = atomicAdd(ret.count, 1);
       if (slot < ret.capacity) lane_store(L, ret.buf + slot);
       atomicAdd(&stats->n[SN_REENTER], 1ull);
