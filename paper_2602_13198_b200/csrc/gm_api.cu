@@ -144,6 +144,7 @@ static void fill_dev_params(gm_ctx* c) {
   P.dx1 = p.dx[1]; P.dx2 = p.dx[2]; P.dx3 = p.dx[3];
   P.inv_dx1 = 1.0 / p.dx[1]; P.inv_dx2 = 1.0 / p.dx[2]; P.inv_dx3 = 1.0 / p.dx[3];
   P.x1lo = p.startx[1]; P.x1hi = p.startx[1] + p.n1 * p.dx[1];
+  P.cell_c1 = -p.startx[1] * P.inv_dx1 - 0.5; P.cell_c2 = -p.startx[2] * P.inv_dx2 - 0.5; P.cell_c3 = -p.startx[3] * P.inv_dx3 - 0.5;
   P.n1 = p.n1; P.n2 = p.n2; P.n3 = p.n3; P.metric_kind = p.metric_kind;
   P.L_unit = p.L_unit;
   P.T_unit = p.L_unit / C_CL;

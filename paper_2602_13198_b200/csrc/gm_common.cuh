@@ -39,6 +39,7 @@ struct DevParams {
   double a_spin, hslope;
   double startx1, startx2, startx3, dx1, dx2, dx3, inv_dx1, inv_dx2, inv_dx3;
   double x1lo, x1hi;
+  double cell_c1, cell_c2, cell_c3;                   // -startx/dx - 1/2: stencil index of a coordinate as one FMA (cell_index)
   int n1, n2, n3, metric_kind;
   // units
   double L_unit, T_unit, B_unit, Ne_unit, Cfac;       // Cfac = h L_unit/(m_e c^2)

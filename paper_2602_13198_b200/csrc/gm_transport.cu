@@ -410,19 +410,22 @@ __device__ __forceinline__ bool stop_tests(const DevParams& P, Lane& L, const Ta
 // length zero (mode 3): the ordinary gather / plasma / opacity code, all lanes of the warp busy with their own steps,
 // forms the exact (nua_s, bias) at the record's point; then it continues as usual.  Every decision is the one the
 // exact evaluation takes, so no history changes (the parity tests compare them one by one).
+// Index of the interpolation cell of a point = index of the cell's lowest corner zone (axis_weights of interp_prim,
+// with the offset folded into one FMA per axis: where the two roundings disagree the point sits on the face between
+// two cells to 1e-16, the interpolant there is the shared corners' to the same accuracy, and the bounds of either
+// cell hold with their 1e-6 margin).
 template <bool THREED>
 __device__ __forceinline__ long cell_index(const DevParams& P, const double x[4]) {
-  int i0, i1, j0, j1;
-  double w;
-  axis_weights(x[1], P.startx1, P.inv_dx1, P.n1, i0, i1, w);
-  double x2 = x[2];
-  if (x2 < 0.0) x2 = -x2;
+  int i0 = 0, j0 = 0;
+  if (P.n1 > 1) i0 = min(max((int)fma(x[1], P.inv_dx1, P.cell_c1), 0), P.n1 - 2);
+  double x2 = fabs(x[2]);
   if (x2 > 1.0) x2 = 2.0 - x2;
-  axis_weights(x2, P.startx2, P.inv_dx2, P.n2, j0, j1, w);
-  long z = ((long)i0 * P.n2 + j0) * P.n3;
+  if (P.n2 > 1) j0 = min(max((int)fma(x2, P.inv_dx2, P.cell_c2), 0), P.n2 - 2);
+  int z = (i0 * P.n2 + j0) * P.n3;                        // (zones < 2^31: the run buffers index them with int too)
   if (THREED) {
-    const long kk = (long)floor((x[3] - P.startx3) * P.inv_dx3 - 0.5), n3 = P.n3;
-    z += ((kk % n3) + n3) % n3;
+    int k0 = (int)floor(fma(x[3], P.inv_dx3, P.cell_c3)) % P.n3;
+    if (k0 < 0) k0 += P.n3;
+    z += k0;
   }
   return z;
 }
@@ -431,7 +434,7 @@ __device__ __forceinline__ long cell_index(const DevParams& P, const double x[4]
 #define GM_TRACK_MINBLOCKS 3
 #endif
 #ifndef GM_COLD_MINBLOCKS
-#define GM_COLD_MINBLOCKS GM_TRACK_MINBLOCKS
+#define GM_COLD_MINBLOCKS 4                 // cold pass (bounded steps only): 128 registers, 16 warps per SM
 #endif
 
 template <bool KERR, bool THREED, int PHASE>
@@ -461,6 +464,8 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
   L.id0 = L.id1 = L.id2 = L.nstep = L.jscat = 0u; L.nsc = 0; L.root = -1; L.flags = 0;
 #pragma unroll
   for (int m = 0; m < 4; m++) { L.x[m] = 0.0; L.k[m] = 0.0; L.a[m] = 0.0; }
+  __shared__ uint4 s_cb[TRACK_WARPS][32];                 // cold pass: the cell bounds of each lane's end point
+  uint4* const stage_cb = s_cb[wid];
   bool have = false;
   int ncold = 0;                        // PHASE_HOT: consecutive committed cold steps of this lane
   int mode = 0;                         // 0 normal step, 1 partial push to a scattering event, 2 redo full step
@@ -543,7 +548,10 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
         if (slot < esc.capacity) lane_store(L, esc.buf + slot);
         have = false; continue;
       }
-      double ur;
+      double ur = 0.0;
+      // cold pass: the uniform of the scattering test is drawn after the push (nothing of it lives across the Verlet
+      // loop); the roulette uniform of the same block only for the few superphotons below w_min
+      if (PHASE != PHASE_COLD || L.w < P.w_min)
       uniform_pair(P, TAG_STEP, L.id0, L.id1, L.id2, L.nstep, ux, ur);
       if (L.w < P.w_min && !(L.flags & FLAG_ROULETTED)) {
         // most roulettes kill (survival 1/roulette): counted in registers, no call and no lane copy unless a
@@ -575,8 +583,16 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
     if (PHASE == PHASE_COLD) {
       const bool ingrid = x1[1] >= P.x1lo && x1[1] < P.x1hi;
       double2 cb = make_double2(0.0, 0.0);
-      if (ingrid) cb = __ldg(P.cellB + cell_index<THREED>(P, x1));      // flies during the push
+      // the cell's bounds fly into the lane's shared-memory slot during the push (no register held)
+      if (ingrid) {
+        const unsigned d = (unsigned)__cvta_generic_to_shared(stage_cb + lane);
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(d), "l"(P.cellB + cell_index<THREED>(P, x1)));
+      }
+      asm volatile("cp.async.commit_group;");
       it = push_wavevector<KERR>(P, L.k, L.a, dl_eff, x1, k1, a1, G, capped);
+      asm volatile("cp.async.wait_group 0;" ::: "memory");
+      if (ingrid) cb = *reinterpret_cast<const double2*>(stage_cb + lane);
+      { double ur2; uniform_pair(P, TAG_STEP, L.id0, L.id1, L.id2, L.nstep, ux, ur2); }
       bool decided = !ingrid;                              // beyond the grid: vacuum, (0, 1) exactly
       if (ingrid && cb.y < P.thetae_min && k1[0] > 0.0) {  // certainly not hot: the cell's bounds stand in
         decided = true; bnd1 = true;
