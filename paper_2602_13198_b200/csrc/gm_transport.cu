@@ -205,6 +205,9 @@ __global__ void __launch_bounds__(128, GM_EMIT_MINBLOCKS) emit_kernel(const DevP
 // A history is a pure function of its record (counter-based RNG), so the passes change no result.
 // =====================================================================================================
 constexpr int PHASE_MIXED = 0, PHASE_HOT = 1, PHASE_COLD = 2;
+#ifndef GM_SMALL_PASS
+#define GM_SMALL_PASS 262144
+#endif
 #ifndef GM_QUIET_BT
 #define GM_QUIET_BT (1.0 / 64.0)
 #endif
@@ -455,6 +458,9 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
   // every queue is checked by its consumer: a producer that ran past the capacity dropped records, which the host
   // must hear about (sticky flag, read back by run_batch; "nothing is dropped silently")
   if (blockIdx.x == 0 && threadIdx.x == 0 && *in_count > in_capacity) atomicOr(overflow, 1);
+  // a hot pass whose input would not fill the machine (less than one superphoton per resident lane) keeps its
+  // superphotons to the end: every further pass would be a launch that waits for a few long histories
+  const int k_cold_eff = (PHASE == PHASE_HOT && n_in < GM_SMALL_PASS) ? 0x7fffffff : k_cold;
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const unsigned lt_mask = (1u << lane) - 1u;
   uint4* stage = s_dyn + wid * (STAGE_REC * PH_U4);
@@ -697,7 +703,7 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
     mode = 0;
     if (PHASE == PHASE_HOT) {
       ncold = (hot || !quiet) ? 0 : ncold + 1;             // quiet: a step the cold pass could have decided with its bounds
-      if (ncold >= k_cold && L.x[1] < P.x1hi) {            // cold for k_cold steps: continue in the cold pass
+      if (ncold >= k_cold_eff && L.x[1] < P.x1hi) {            // cold for k_cold steps: continue in the cold pass
         const int slot = atomicAdd(park.count, 1);
         if (slot < park.capacity) lane_store(L, park.buf + slot);
         have = false;
