@@ -125,7 +125,10 @@ enum { GM_EVAL_ACCEL = 0,   /* in x[4],k[4]            -> out a[4] = -Gamma^m_ab
        GM_EVAL_OPAC = 3,    /* in x[4],k[4]            -> out nu*alpha_abs, nu*alpha_scat, bias (nsc=0) */
        GM_EVAL_PUSH = 4,    /* in x[4],k[4],a[4],dl    -> out x[4],k[4],a[4],iters (Eq. 11-15)          */
        GM_EVAL_RAD = 5,     /* in nu,ne,thetae,B,sin   -> out j_nu (Eq. 3), nu*alpha (Eq. 16/20), sigma_h/sigma_T(thetae, h nu/m c^2) */
-       GM_EVAL_NB = 6       /* in x                    -> out the hot loop's branch-free 1/x, sqrt(x), exp(x) */ };
+       GM_EVAL_NB = 6,      /* in x                    -> out the hot loop's branch-free 1/x, sqrt(x), exp(x) */
+       GM_EVAL_BOUND = 7    /* in x[4],k[4] (after gm_prepare) -> out k^t S, Theta_B of the point's interpolation cell (the cold
+                               pass's upper bounds), then the exact nu*alpha_scat, Theta_e, bias(Theta_B),
+                               bias(Theta_e) at the point (nsc = 0) */ };
 
 typedef struct gm_ctx gm_ctx; /* opaque; owned by the library */
 

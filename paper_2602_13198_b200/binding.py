@@ -17,9 +17,9 @@ LIB_PATH = os.environ.get("GPUMONTY_B200_LIB") or os.path.join(_HERE, "libgpumon
 
 GM_ABI_VERSION = 2
 TABLE_LNK2, TABLE_LNF, TABLE_LNSIGH, TABLE_LNW, TABLE_NEXP, TABLE_QMAX = range(6)
-EVAL_ACCEL, EVAL_GEOM, EVAL_PLASMA, EVAL_OPAC, EVAL_PUSH, EVAL_RAD, EVAL_NB = range(7)
+EVAL_ACCEL, EVAL_GEOM, EVAL_PLASMA, EVAL_OPAC, EVAL_PUSH, EVAL_RAD, EVAL_NB, EVAL_BOUND = range(8)
 _EVAL_SHAPES = {EVAL_ACCEL: (8, 4), EVAL_GEOM: (4, 33), EVAL_PLASMA: (4, 12), EVAL_OPAC: (8, 3),
-                EVAL_PUSH: (13, 13), EVAL_RAD: (5, 3), EVAL_NB: (1, 3)}
+                EVAL_PUSH: (13, 13), EVAL_RAD: (5, 3), EVAL_NB: (1, 3), EVAL_BOUND: (8, 6)}
 FATE_ALIVE, FATE_RECORDED, FATE_HORIZON, FATE_ROULETTE, FATE_MAXSTEP, FATE_OUTOFRANGE, FATE_ANALOG = range(7)
 
 EXPORTS = ["gm_create", "gm_destroy", "gm_last_error", "gm_set_grid", "gm_prepare", "gm_get_zone_counts",

@@ -768,9 +768,10 @@ int gm_trace(gm_ctx* ctx, const int64_t* ids, int n, gm_trace_rec* out) {
 
 int gm_eval(gm_ctx* ctx, int what, const double* in, int n, double* out) {
   if (!ctx || !in || !out || n < 0) return GM_ERR_PARAM;
-  static const int nin[] = {8, 4, 4, 8, 13, 5, 1}, nout[] = {4, 33, 12, 3, 13, 3, 3};
-  if (what < 0 || what > GM_EVAL_NB) return fail(ctx, GM_ERR_PARAM, "unknown eval %d", what);
+  static const int nin[] = {8, 4, 4, 8, 13, 5, 1, 8}, nout[] = {4, 33, 12, 3, 13, 3, 3, 6};
+  if (what < 0 || what > GM_EVAL_BOUND) return fail(ctx, GM_ERR_PARAM, "unknown eval %d", what);
   if ((what == GM_EVAL_PLASMA || what == GM_EVAL_OPAC) && !ctx->have_grid) return fail(ctx, GM_ERR_STATE, "no grid");
+  if (what == GM_EVAL_BOUND && !ctx->prepared) return fail(ctx, GM_ERR_STATE, "not prepared");
   if (n == 0) return GM_OK;
   double *d_in = nullptr, *d_out = nullptr;
   CK(cudaMalloc((void**)&d_in, (size_t)n * nin[what] * sizeof(double)));

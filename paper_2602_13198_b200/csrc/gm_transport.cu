@@ -1186,6 +1186,23 @@ __global__ void eval_kernel(const DevParams P, int what, const double* __restric
     out[3 * i] = jnu_K2(r[0], r[1], r[2], r[3], r[4], K2_eval(P, r[2]));
     out[3 * i + 1] = nu_alpha_abs(P, r[0], r[1], r[2], r[3], r[4]);
     out[3 * i + 2] = P.lnSigH ? sigma_hot_eval(P, r[2], r[0] * C_H_MEC2) : 0.0;
+  } else if (what == GM_EVAL_BOUND) {
+    const double* r = in + 8 * i;
+    double* o = out + 6 * i;
+    for (int m = 0; m < 6; m++) o[m] = 0.0;
+    o[4] = o[5] = 1.0;
+    if (r[1] >= P.x1lo && r[1] < P.x1hi) {
+      const double2 cb = P.cellB[cell_index<THREED>(P, r)];
+      o[0] = r[4] * cb.x; o[1] = cb.y; o[4] = bias_func(P, cb.y, 0);
+      Geom G;
+      geom_at<KERR, false>(P, r[1], r[2], G, nullptr);
+      Plasma S;
+      if (plasma_at<THREED>(P, r, G, S)) {
+        double na, ns, b;
+        opacities<false>(P, r + 4, G, S, 0, P.scattering_on != 0, na, ns, b);
+        o[2] = ns; o[3] = S.thetae; o[5] = b;
+      }
+    }
   } else if (what == GM_EVAL_NB) {
     out[3 * i] = rcp_nb(in[i]); out[3 * i + 1] = sqrt_nb(in[i]); out[3 * i + 2] = exp_nb(in[i]);
   }

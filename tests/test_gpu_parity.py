@@ -151,6 +151,65 @@ def test_geometry_accel_plasma_opacity_push(gm, olib, cfg):
     assert np.all(np.isfinite(OP)) and np.any(OP[:, 1] > 0)
 
 
+@pytest.mark.parametrize("cfg", ["kerr", "kerr_dense", "kerr3d"])
+def test_cold_pass_bounds_dominate_the_exact_plasma_state(gm, olib, cfg):
+    """DESIGN.md section 6 "bounded steps": the cold tracker pass decides its scattering test and rules out absorption
+    with per-cell upper bounds (cell_bound_kernel) instead of the plasma state.  That changes no history only if the
+    bounds really are upper bounds EVERYWHERE in the cell: k^t S >= nu alpha_s, Theta_B >= Theta_e, b(Theta_B) >= b
+    for any point and any future-directed null wavevector -- checked here on random points (cell interiors, the half
+    zones beyond the outermost centres, next to the polar axis and across it) against the exact evaluation of the CUDA
+    path and against the oracle's plasma state, and that the bounds are tight enough to be of use away from the torus."""
+    rng = np.random.default_rng(5)
+    if cfg == "kerr":
+        p, prim = wl.config2(Ns=1e3, n1=64, n2=64)
+    elif cfg == "kerr_dense":
+        p, prim = wl.config4(Ns=1e3, n1=96, n2=48)
+    else:
+        p, prim = wl.config3(Ns=1e3, n1=24, n2=16, n3=16)
+    o, g = _pair(gm, p, prim, prepare=True)
+    n = 6000
+    x = _points(p, n, rng, inside=True)
+    lo, hi = p["startx"][1], p["startx"][1] + p["n1"] * p["dx"][1]
+    x[: n // 6, 1] = rng.uniform(hi - 0.6 * p["dx"][1], hi - 1e-9, n // 6)            # last half zone
+    x[n // 6: n // 3, 1] = rng.uniform(lo, lo + 4 * p["dx"][1], n // 6)
+    x[n // 3: n // 2, 2] = rng.choice([-1.0, 1.0], n // 6) * rng.uniform(-0.01, 0.02, n // 6) % 1.0   # around the axis
+    x[n // 2: n // 2 + 200, 2] = rng.uniform(-0.02, 0.0, 200)                           # beyond it (G33)
+    x[:, 1] = np.maximum(x[:, 1], math.log(1.45))                                       # outside the horizon
+    # future-directed null wavevectors from the oracle's metric: random spatial part, k^t from k.k = 0
+    k = rng.normal(size=(n, 4))
+    k[:, 1] /= np.exp(x[:, 1]); k[:, 2] /= np.exp(x[:, 1]) * 3; k[:, 3] /= np.exp(x[:, 1])
+    for i in range(n):
+        gc = olib.gcov(o.P, x[i])
+        a, b = gc[0, 0], gc[0, 1:] @ k[i, 1:]
+        c = k[i, 1:] @ gc[1:, 1:] @ k[i, 1:]
+        disc = b * b - a * c
+        if a > 0 and (b > 0 or disc < 0):      # inside the ergosphere every future-directed null vector co-rotates
+            k[i, 1:] = -k[i, 1:]; b = -b
+            if disc < 0:
+                k[i, 1:3] = 0.0; b = gc[0, 3] * k[i, 3]; c = gc[3, 3] * k[i, 3] ** 2; disc = b * b - a * c
+        k[i, 0] = max((-b + math.sqrt(max(disc, 0.0))) / a, (-b - math.sqrt(max(disc, 0.0))) / a)
+    ok = k[:, 0] > 0
+    assert np.count_nonzero(ok) > 0.9 * n             # (the rest: no null vector found next to the horizon)
+    x, k = x[ok], k[ok]
+    n = len(x)
+    k *= 1e-9                                                                           # ~1e11 Hz
+    B = g.eval(gm.EVAL_BOUND, np.hstack([x, k]))
+    nsB, thB, ns, th, bB, b = B.T
+    assert np.all(nsB >= ns) and np.all(thB >= th) and np.all(bB >= b)
+    assert np.count_nonzero(ns > 0) > 0.9 * n
+    # against the oracle's own plasma state (independent code)
+    for i in range(0, n, 40):
+        ref = o.plasma_at(x[i])
+        if not ref["vacuum"]:
+            assert thB[i] >= ref["thetae"]
+    # usefulness: away from the magnetised torus the bounds stay within a small factor of the exact values
+    cold = (thB < p["thetae_min"]) & (ns > 0)
+    assert np.count_nonzero(cold) > 0.3 * n
+    assert np.median(nsB[cold] / ns[cold]) < 20.0 and np.median(thB[cold] / np.maximum(th[cold], 1e-300)) < 3.0
+    print("\nbounds (%s): %d of %d points certainly cold; median k^t S / (nu alpha_s) %.2f, Theta_B / Theta_e %.3f"
+          % (cfg, np.count_nonzero(cold), n, np.median(nsB[cold] / ns[cold]), np.median(thB[cold] / th[cold])))
+
+
 def test_radiation_functions(gm, olib):
     p, prim = wl.config1(Ns=1e3)
     g = gm.GPUMonty(p)
