@@ -35,19 +35,22 @@ from paper_2602_13198_b200.shard import rank_seed, reduce_tally  # noqa: E402
 
 METRIC = "superphotons/s tracked (incl. scattering)"
 UNIT = "superphotons/s"
-# algorithmic FP64 flop per geodesic step (dadd + dmul + 2 dfma predicated-on thread
-# instructions of the kernel divided by the steps it committed, counted with ncu on each workload class with the
-# single mixed tracker pass, so that no redone step is counted -- profiles/r02_final.md, r02j_flops_cfg*.csv -- and
-# then frozen).  "track": in-grid step of track_kernel; "escape": free-flight step of escape_kernel.
-FLOP_PER_STEP = {"flat": {"track": 705.8, "escape": 208.0}, "kerr": {"track": 693.7, "escape": 368.2},
-                 "kerr3d": {"track": 808.5, "escape": 368.2}}
-# dram__bytes_read.sum + dram__bytes_write.sum of the dominant launch from one ncu --set full capture; a constant of
-# that capture (its command and N_s are named in TRAFFIC_SOURCE), not a quantity measured in this run.  The run
-# itself reports the ALGORITHMIC bytes per launch beside it (roofline.algorithmic_bytes_per_launch).
-TRAFFIC_BYTES_PER_LAUNCH = {2: 274.7e6 + 364.2e6}
-TRAFFIC_SOURCE = {2: "profiles/r02_final.md (ncu --set full of this workload, cfg2 at N_s=1e7): first cold tracker pass, "
-                     "11.8 ms under ncu; reads the 1.7e6 records the hot pass parked, writes 2.3e6 hand-over / free-flight / "
-                     "scattered records of 160 B: DRAM traffic = algorithmic record bytes, the gather is served by L1/L2"}
+# algorithmic FP64 flop per geodesic step: dadd + dmul + 2 dfma predicated-on thread instructions
+# of ALL tracker launches of a step divided by the in-grid steps they committed, counted with ncu on each config at
+# the N_s and with the pass schedule this file times (profiles/r02_final.md, r02_flops_cfg*.csv), then frozen.  Since
+# round 2 the figure depends on the config: a bounded step of the cold pass (configs 2, 3) needs neither gather nor
+# plasma state nor opacity, a step in hot plasma needs all of them.  "track": average over the in-grid steps of
+# track_kernel (all passes); "escape": free-flight step of escape_kernel.
+FLOP_PER_STEP = {0: {"track": 681.1, "escape": 208.4}, 1: {"track": 705.8, "escape": 208.4},
+                 2: {"track": 516.3, "escape": 368.2}, 3: {"track": 560.0, "escape": 368.2},
+                 4: {"track": 700.3, "escape": 368.2}}
+# dram__bytes_read.sum + dram__bytes_write.sum of the dominant launch from one ncu capture; a constant of that capture
+# (its command and N_s are named in TRAFFIC_SOURCE), not a quantity measured in this run.  The run itself reports the
+# ALGORITHMIC bytes per launch beside it (roofline.algorithmic_bytes_per_launch).
+TRAFFIC_BYTES_PER_LAUNCH = {2: 2.897e9 + 2.832e9}
+TRAFFIC_SOURCE = {2: "profiles/r02_final.md (ncu --set full of this workload, cfg2 at N_s=1e7): hot tracker pass of the largest "
+                     "scattering generation, 59 ms: reads 1.6e7 records of 160 B, writes as many hand-over / free-flight / "
+                     "scattered records: DRAM traffic = algorithmic record bytes, the gather is served by L1/L2"}
 WORKLOAD_NAMES = {0: "cfg0 thin synchrotron sphere 32x16, Ns=1e5", 1: "cfg1 scattering sphere 32x16, Ns=1e6",
                   2: "cfg2 Kerr FM torus 256x256, Ns=1e7", 3: "cfg3 3-D perturbed torus 192x128x128, Ns=1e7",
                   4: "cfg4 Kerr torus x1e3 density (analog scattering), Ns=1e6"}
@@ -244,12 +247,11 @@ def main():
         ms_step, ms_step_e2e = float(t_dev[0]), float(t_dev[1])
         total = float(cnt[0])
         value = total / (ms_step * 1e-3)
-        kind = ("kerr3d" if p["n3"] > 1 else "kerr") if p["metric_kind"] == 1 else "flat"
         n_track_launches = max(1, tm["track"][1])
         steps_track = st["n_steps_total"] - st["n_steps_free"]      # steps taken inside track_kernel (this rank, last timed step)
-        flops = steps_track * FLOP_PER_STEP[kind]["track"]
+        flops = steps_track * FLOP_PER_STEP[cfg]["track"]
         esc_ms = tm["escape"][0] / steps
-        esc_tflops = st["n_steps_free"] * FLOP_PER_STEP[kind]["escape"] / max(esc_ms * 1e-3, 1e-9) / 1e12
+        esc_tflops = st["n_steps_free"] * FLOP_PER_STEP[cfg]["escape"] / max(esc_ms * 1e-3, 1e-9) / 1e12
         track_ms_per_step = tm["track"][0] / steps
         achieved = flops / (track_ms_per_step * 1e-3) / 1e12
         launches = sum(v[1] for v in tm.values()) // max(1, steps)
@@ -276,9 +278,9 @@ def main():
                          "traffic_source": TRAFFIC_SOURCE.get(cfg),
                          "algorithmic_bytes_per_launch": alg_bytes,
                          "peak_source": "DFMA-chain microbenchmark run in this process (gm_fp64_peak); nominal 2*64*148*1.965 GHz = 37.2",
-                         "flop_per_step": FLOP_PER_STEP[kind]["track"], "track_ms_per_step": track_ms_per_step,
+                         "flop_per_step": FLOP_PER_STEP[cfg]["track"], "track_ms_per_step": track_ms_per_step,
                          "escape_kernel": {"achieved": esc_tflops, "frac": esc_tflops / peak, "ms_per_step": esc_ms,
-                                           "flop_per_step": FLOP_PER_STEP[kind]["escape"]},
+                                           "flop_per_step": FLOP_PER_STEP[cfg]["escape"]},
                          "track_launches_per_step": lpl,
                          "track_share_of_step": track_ms_per_step / ms_step,
                          "kernel_ms_per_step": {k: v[0] / steps for k, v in tm.items()}},
