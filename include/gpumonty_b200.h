@@ -42,8 +42,8 @@ enum {
   GM_ERR_GRID = -5      /* non-finite value in the fluid grid            */
 };
 
-/* POD parameter block, copied at gm_create.  Field meaning and defaults: DESIGN.md "Parameters".
- * Same field names as the dict produced by paper_2602_13198_b200.workloads. */
+/* POD parameter block, copied at gm_create.  Field meaning: the comments below and DESIGN.md section 2 (readings G0-G33);
+ * the values of the five configs: DESIGN.md section 4.  Same field names as the dict produced by paper_2602_13198_b200.workloads. */
 typedef struct gm_params {
   uint32_t abi_version;      /* must equal GM_ABI_VERSION                                            */
   int32_t metric_kind;       /* 0 flat (Kerr-Schild form with M = 0), 1 Kerr-Schild M = 1            */
