@@ -279,6 +279,8 @@ def main():
                          "algorithmic_bytes_per_launch": alg_bytes,
                          "peak_source": "DFMA-chain microbenchmark run in this process (gm_fp64_peak); nominal 2*64*148*1.965 GHz = 37.2",
                          "flop_per_step": FLOP_PER_STEP[cfg]["track"], "track_ms_per_step": track_ms_per_step,
+                         "flop_per_step_note": "algorithmic flop of THIS implementation (ncu-counted, profiles/r02_final.md); "
+                                               "round 1 needed 693.7 (cfg2) / 808.5 (cfg3) per step for the same histories",
                          "escape_kernel": {"achieved": esc_tflops, "frac": esc_tflops / peak, "ms_per_step": esc_ms,
                                            "flop_per_step": FLOP_PER_STEP[cfg]["escape"]},
                          "track_launches_per_step": lpl,
