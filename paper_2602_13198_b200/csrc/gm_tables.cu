@@ -347,7 +347,7 @@ __global__ void __launch_bounds__(256) scan_tile_kernel(const int32_t* __restric
 //                                            gamma (1 + v) = gamma + sqrt(gamma^2 - 1), rising with gamma;
 //   sigma_h / sigma_T                       <= 1.
 // So nu alpha_s <= k^t S with S = (gamma_B + sqrt(gamma_B^2 - 1)) n_e,B sigma_T m_e c^2/h, and the bias b(Theta_e) <= b(Theta_B) (G21 is
-// non-decreasing in Theta_e).  Each bound carries a margin of 1e-6 against the rounding of the exact evaluation.
+// non-decreasing in Theta_e).  Theta_B carries a margin of 1e-6 against the rounding of the exact evaluation, S one of 1 %.
 // A cell whose state cannot be bounded (non-finite input, u > 0 on rho = 0) gets Theta_B = inf: never skipped.
 template <bool KERR>
 __global__ void cell_bound_kernel(const DevParams P, double2* __restrict__ cellB, long nz) {
@@ -389,7 +389,9 @@ __global__ void cell_bound_kernel(const DevParams P, double2* __restrict__ cellB
   }
   thB = fmin(thB * (1.0 + 1e-6), P.thetae_max);
   const double gamB = sqrt(1.0 + 100.0 * q_max);
-  double S = (gamB + sqrt(100.0 * q_max)) * (rho_max * P.Ne_unit) * C_SIGT * C_MEC2_H * (1.0 + 1e-6);
+  // (x 1.01: the decomposition k = E_n (n + n^) assumes a null k; the integrated k.k drifts from 0 by a small multiple of
+  // verlet_tol, which lets the spatial part exceed E_n by that much)
+  double S = (gamB + sqrt(100.0 * q_max)) * (rho_max * P.Ne_unit) * C_SIGT * C_MEC2_H * 1.01;
   if (!ok || !isfinite(S) || !isfinite(thB)) { S = INFINITY; thB = INFINITY; }
   cellB[z] = make_double2(S, thB);
 }
