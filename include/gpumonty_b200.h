@@ -165,13 +165,15 @@ int gm_run(gm_ctx* ctx, int64_t first_id, int64_t n_ids, void* cuda_stream);
  * (records).  0 keeps the default.  Call before the first gm_run. */
 int gm_set_batch(gm_ctx* ctx, int64_t batch_primaries, int64_t queue_records);
 /* Tracker schedule (a tuning knob; no result depends on it).  Absorption (PAPER.md:114-140,
- * Eq. 16-20) is evaluated only where Theta_e >= thetae_min; each scattering generation can therefore be tracked in
- * `pairs` hot/cold pass pairs: a hot pass hands a superphoton over after `k_cold` consecutive cold steps, a cold
- * pass hands it back when it meets hot plasma, the last cold pass handles hot plasma in place.  pairs = 0: one
- * mixed pass; pairs > 0 is honoured for metric_kind = 1 only; pairs < 0 (default): automatic -- none for batches
- * below 5e5 primaries or a uniform Theta_e; otherwise the first hot pass of the first batch of >= 1e6 primaries
- * after gm_prepare is run, and 2 pairs are used from then on if it handed over >= 0.35 of its primaries, else
- * none.  k_cold >= 1.  Call before the first gm_run (run buffers are re-allocated). */
+ * Eq. 16-20) is evaluated only where Theta_e >= thetae_min, and the scattering test can be decided far
+ * from the torus with per-cell upper bounds; each scattering generation can therefore be tracked in `pairs` hot/cold
+ * pass pairs: a hot pass (the full step) hands a superphoton over after `k_cold` consecutive quiet steps (not in hot
+ * plasma, b tau_s < 1/64), a cold pass takes only steps its bounds decide and hands everything else back, a last
+ * mixed pass does everything in place.  pairs = 0: one mixed pass; pairs > 0 is honoured for metric_kind = 1 only;
+ * pairs < 0 (default): automatic -- none for batches below 5e5 primaries or a uniform Theta_e; otherwise the first
+ * hot pass of the first batch of >= 1e6 primaries after gm_prepare is run, and 3 pairs are used from then on if it
+ * handed over >= 0.35 of its primaries, else none.  k_cold >= 1.  Call before the first gm_run (run buffers are
+ * re-allocated). */
 int gm_set_phase_passes(gm_ctx* ctx, int pairs, int k_cold);
 
 /* Bias tuning (262-264, 304; G32).  With gm_params.bias_tune = 1, gm_prepare tunes one factor per

@@ -198,9 +198,10 @@ __global__ void __launch_bounds__(128, GM_EMIT_MINBLOCKS) emit_kernel(const DevP
 // plasma with Theta_e >= thetae_min -- in the torus workloads 13 % of the in-grid steps, mostly at the start of a
 // history (superphotons are emitted and scattered where the plasma is hot).  With young and old histories mixed
 // in one warp that block runs at 4 of 32 lanes in nearly every iteration.  So a generation is tracked in passes:
-//   PHASE_HOT   a lane whose last `k_cold` committed steps were all cold stores its state to the `park` queue;
-//   PHASE_COLD  a lane that meets hot plasma stores its start-of-step state to `park` (the step is redone by
-//               the next hot pass; nothing of the absorption block is executed in this pass);
+//   PHASE_HOT   the full step; a lane whose last `k_cold` committed steps were all QUIET (not in hot plasma and
+//               b tau_s < GM_QUIET_BT) stores its state to the `park` queue -- unless the launch's input is small;
+//   PHASE_COLD  bounded steps only ("bounded steps of the cold pass" below: no gather, no plasma state, no
+//               opacity); a lane whose next step the bounds do not decide stores its start-of-step state to `park`;
 //   PHASE_MIXED everything in place (the last pass of a generation, and every pass of the flat workloads).
 // A history is a pure function of its record (counter-based RNG), so the passes change no result.
 // =====================================================================================================
