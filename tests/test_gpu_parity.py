@@ -540,8 +540,10 @@ def test_subzone_emission_positions(gm, cfg):
     _compare_traces(o, g, np.arange(0, g.n_primaries, 11), fork_budget=2e-4)
 
 
-@pytest.mark.parametrize("cfg,pairs,k_cold", [(2, 1, 1), (2, 2, 4), (2, 3, 2), (3, 2, 3), (4, 2, 1)])
-def test_hot_cold_phase_passes_change_no_history(gm, cfg, pairs, k_cold):
+@pytest.mark.parametrize("cfg,pairs,k_cold,variant", [
+    (2, 1, 1, ""), (2, 2, 4, ""), (2, 3, 2, ""), (3, 2, 3, ""), (4, 2, 1, ""), (3, 3, 4, ""),
+    (2, 3, 4, "thetae_mode1"), (2, 2, 4, "no_scattering"), (2, 3, 3, "subzone_tuned_bias"), (4, 3, 4, "unfolded_nsc2")])
+def test_hot_cold_phase_passes_change_no_history(gm, cfg, pairs, k_cold, variant):
     """Tracker schedule (gm_set_phase_passes): a history is a pure function of its record, so
     handing superphotons between hot and cold passes must leave every counter and every bin count unchanged
     (sums differ only by the order of the fp64 atomics).  The forced schedule is also compared with the oracle."""
@@ -551,6 +553,15 @@ def test_hot_cold_phase_passes_change_no_history(gm, cfg, pairs, k_cold):
         p, prim = wl.config3(Ns=1e4, n1=48, n2=32, n3=32)
     else:
         p, prim = wl.config4(Ns=5e3)
+    # other parameter regimes of the same grids (the cold pass's bounds depend on the Theta_e prescription and the bias law)
+    if variant == "thetae_mode1":
+        p.update(thetae_mode=1, trat=3.0, bias0=20.0)    # (hotter electrons: the calibrated bias0 would overflow the queue)
+    elif variant == "no_scattering":
+        p.update(scattering_on=0)
+    elif variant == "subzone_tuned_bias":
+        p.update(emit_mode=1, bias_tune=1, bias0=1.0, bias_target=3.0)
+    elif variant == "unfolded_nsc2":
+        p.update(fold_theta=0, nsc_max=2, bias0=30.0, bias_p_theta=1, bias_q_nsc=1)
     res = []
     for pr_ in (0, pairs):
         g = gm.GPUMonty(p)
