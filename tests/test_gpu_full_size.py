@@ -103,6 +103,11 @@ def test_full_size_spectrum_against_the_stored_oracle_tally(gm, cfg):
     p, prim = wl.CONFIGS[cfg](**FULL_SIZE[cfg])
     gold = _golden(cfg, p)
     g = gm.GPUMonty(p)
+    if cfg == 3:
+        # the stored tally is at N_s = 1e6 (382k primaries), below the size at which the automatic schedule uses the
+        # hot / bounded-cold passes: force them, so that the 3.1e6-cell bound table of the full grid is exercised too
+        # (cfg 2 at its 3.6e6 primaries gets them by itself)
+        g.set_phase_passes(3, 4)
     g.set_grid(prim)
     n = g.prepare()
     assert n == int(gold["n_primaries"])
