@@ -499,6 +499,13 @@ static int run_batch(gm_ctx* ctx, long long first, int n, const long long* d_ids
             if (ctx->auto_pairs == 0) pairs = 1;           // finish this generation with the mixed pass, then none
           }
           if (pp >= pairs - 1) {
+            // what the last hot pass handed over is mostly quiet: one more cold pass takes the steps its bounds decide,
+            // the mixed pass finishes the rest in place
+            if (pairs > 1) {
+              CK(cudaMemsetAsync(parkB.count, 0, sizeof(int), st));
+              TIMED(GM_T_TRACK, st, launch_track(ctx->P, 2, parkA.buf, parkA.count, parkA.capacity, cnt + 1, out, esc, parkB, 0, carry, tally, stats, trace, oflow, ctx->n_sm, st));
+              TIMED(GM_T_TRACK, st, launch_track(ctx->P, 0, parkB.buf, parkB.count, parkB.capacity, cnt + 1, out, esc, nopark, 0, carry, tally, stats, trace, oflow, ctx->n_sm, st));
+            } else
             TIMED(GM_T_TRACK, st, launch_track(ctx->P, 0, parkA.buf, parkA.count, parkA.capacity, cnt + 1, out, esc, nopark, 0, carry, tally, stats, trace, oflow, ctx->n_sm, st));
           } else {
             CK(cudaMemsetAsync(parkB.count, 0, sizeof(int), st));
