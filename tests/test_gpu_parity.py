@@ -678,6 +678,23 @@ def test_batching_and_queue_overflow_recovery(gm):
     assert st["n_spawned"] == ref_stats["n_spawned"] and st["n_primary"] == ref_stats["n_primary"]
 
 
+def test_batches_with_phase_passes_and_an_overflowing_queue(gm):
+    """The same on the torus with the hot / bounded-cold passes forced: small batches, two gm_run calls into one
+    tally, and a scattered-superphoton queue that overflows (the batch is redone in smaller pieces from the snapshot
+    of the accumulators) give the counts of the single mixed-pass run."""
+    p, prim = wl.config2(Ns=3e4)
+    g = gm.GPUMonty(p); g.set_phase_passes(0, 4); g.set_grid(prim); n = g.prepare(); g.run()
+    ref = g.tally(); ref_stats = g.stats()
+    g2 = gm.GPUMonty(p); g2.set_phase_passes(3, 2); g2.set_grid(prim); g2.prepare()
+    g2.set_batch(2048, 6000)          # ~7 scattered superphotons per primary: 2048 primaries do not fit 6000 records
+    g2.run(0, n // 2); g2.run(n // 2, n - n // 2)
+    got = g2.tally(); st = g2.stats()
+    assert np.array_equal(ref[3], got[3])
+    assert np.max(_relerr(ref[0], got[0], floor=1e-300)) < 1e-11
+    for k in ("n_primary", "n_spawned", "n_recorded", "n_steps_total", "n_steps_free", "n_horizon", "n_roulette_killed"):
+        assert st[k] == ref_stats[k], k
+
+
 @pytest.mark.parametrize("cfg,world", [(1, 2), (2, 3)])
 def test_contexts_on_disjoint_id_ranges_sum_to_the_single_run(gm, cfg, world):
     """The multi-GPU code path of DESIGN.md section 10 on one device: `world` library contexts,
