@@ -29,6 +29,10 @@ struct gm_ctx {
   int* d_counters = nullptr;         // 72 ints, layout in run_batch
   Photon *d_prim_ph = nullptr, *d_qA = nullptr, *d_qB = nullptr, *d_esc = nullptr;
   Photon *d_parkA = nullptr, *d_parkB = nullptr;   // hot/cold pass hand-over queues (esc_records each)
+  Photon* d_wstack = nullptr;                      // per-warp event stacks of the cascade pass (track_wstack_records)
+  bool cascade_overflowed = false, cascade_skip = false;   // the free-flight queue overflowed in a cascade: redo that batch without
+  int cascade_max = -1;                            // a generation with fewer input records starts the cascade (0: never; default: half the
+                                                   // tracker's resident lanes, set in gm_create); GPUMONTY_B200_CASCADE overrides
   int phase_pairs = -1, k_cold = 4;                // -1: automatic (decided by a pilot batch, see gm_run)
   int auto_pairs = -1;                             // the pilot's decision (-1: not taken yet)
   int carry_lanes = 4;                             // straggler hand-over threshold (0: off); GPUMONTY_B200_CARRY overrides
@@ -85,8 +89,8 @@ static int fail(gm_ctx* c, int code, const char* fmt, ...) {
 
 static void free_run_buffers(gm_ctx* c) {
   cudaFree(c->d_prim_ph); cudaFree(c->d_qA); cudaFree(c->d_qB); cudaFree(c->d_esc);
-  cudaFree(c->d_parkA); cudaFree(c->d_parkB);
-  c->d_prim_ph = c->d_qA = c->d_qB = c->d_esc = c->d_parkA = c->d_parkB = nullptr;
+  cudaFree(c->d_parkA); cudaFree(c->d_parkB); cudaFree(c->d_wstack);
+  c->d_prim_ph = c->d_qA = c->d_qB = c->d_esc = c->d_parkA = c->d_parkB = c->d_wstack = nullptr;
   c->batch_primaries = c->queue_records = c->esc_records = 0;
 }
 
@@ -251,6 +255,8 @@ int gm_create(gm_ctx** out, const gm_params* p) {
       return fail(nullptr, GM_ERR_CUDA, "cudaFuncSetAttribute(track_kernel, max dynamic shared memory): %s", m.c_str());
     }
   }
+  ctx->cascade_max = ctx->n_sm * 192;              // half of n_sm x 3 CTAs x 128 lanes: a generation that cannot fill the machine
+  if (const char* e = getenv("GPUMONTY_B200_CASCADE")) ctx->cascade_max = atoi(e) < 0 ? 0 : atoi(e);
   if (const char* e = getenv("GPUMONTY_B200_CARRY")) ctx->carry_lanes = atoi(e) < 0 ? 0 : (atoi(e) > 32 ? 32 : atoi(e));
   // parameter-free tables (S0)
   cudaError_t te = gm_build_tables(ctx, nullptr) == GM_OK ? cudaSuccess : cudaErrorUnknown;
@@ -422,6 +428,8 @@ static int ensure_run_buffers(gm_ctx* ctx, long long n_ids) {
   if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->d_esc, (size_t)esc * sizeof(Photon));
   if (e == cudaSuccess && pairs > 0) e = cudaMalloc((void**)&ctx->d_parkA, (size_t)esc * sizeof(Photon));
   if (e == cudaSuccess && pairs > 0) e = cudaMalloc((void**)&ctx->d_parkB, (size_t)esc * sizeof(Photon));
+  if (e == cudaSuccess && ctx->p.scattering_on && ctx->cascade_max > 0)
+    e = cudaMalloc((void**)&ctx->d_wstack, (size_t)track_wstack_records(ctx->n_sm) * sizeof(Photon));
   if (e != cudaSuccess) {                        // leave no half-allocated state behind (batch_primaries stays 0)
     free_run_buffers(ctx);
     return fail(ctx, GM_ERR_CUDA, "run buffers (%lld primaries, %lld queue records): %s", batch, queue, cudaGetErrorString(e));
@@ -466,6 +474,7 @@ static int run_batch(gm_ctx* ctx, long long first, int n, const long long* d_ids
   Queue parkA{ctx->d_parkA, cnt + 64, (int)ctx->esc_records}, parkB{ctx->d_parkB, cnt + 65, (int)ctx->esc_records};
   int h_counts[NCNT];
   int mq = 0, round = 0;
+  bool cascaded = false;
   for (;;) {
     // generations 0..layers without a host round trip; afterwards only while re-entrants keep a queue non-empty
     // first block: the nominal generations; afterwards one round per host check (re-entrants from free flight and
@@ -518,12 +527,41 @@ static int run_batch(gm_ctx* ctx, long long first, int n, const long long* d_ids
       TIMED(GM_T_COMPTON, st, launch_compton(ctx->P, out, stats, trace, ctx->n_sm, st));
       TIMED(GM_T_ESCAPE, st, launch_escape(ctx->P, esc, cnt + 1, out, tally, stats, trace, oflow, ctx->n_sm, st));
       in = out.buf; in_count = out.count; in_cap = qcap;
+      // Cascade (PHASE_CASCADE): once a generation's input is small, all remaining generations are tracked in one
+      // launch (each warp converts and tracks the events of its own lanes); events that do not fit a warp's stack
+      // arrive in the next queue and are handled by ordinary rounds.  One 4-byte read-back per generation decides.
+      if (ctx->d_wstack && !ctx->cascade_skip && ctx->p.metric_kind == 1 && first_block && round >= 1 && round < last && round + 2 < MAXROUND) {
+        int n_next = 0;
+        CK(cudaMemcpyAsync(&n_next, out.count, sizeof(int), cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        if (n_next > 0 && n_next <= qcap && n_next < ctx->cascade_max) {
+          round++;
+          Queue out2{(round & 1) ? ctx->d_qB : ctx->d_qA, cnt + 3 + round, qcap};
+          Queue wst{ctx->d_wstack, cnt + 66, track_wstack_per_warp()};
+          CK(cudaMemsetAsync(esc.count, 0, sizeof(int), st));
+          TIMED(GM_T_TRACK, st, launch_track(ctx->P, 3, in, in_count, in_cap, cnt + 1, out2, esc, wst, 0, 0, tally, stats, trace, oflow_in, ctx->n_sm, st));
+          TIMED(GM_T_COMPTON, st, launch_compton(ctx->P, out2, stats, trace, ctx->n_sm, st));
+          TIMED(GM_T_ESCAPE, st, launch_escape(ctx->P, esc, cnt + 1, out2, tally, stats, trace, oflow, ctx->n_sm, st));
+          in = out2.buf; in_count = out2.count; in_cap = qcap;
+          round++;
+          cascaded = true;
+          break;
+        }
+      }
     }
     CK(cudaMemcpyAsync(h_counts, cnt, NCNT * sizeof(int), cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
     for (int r = 0; r < round; r++) if (h_counts[3 + r] > mq) mq = h_counts[3 + r];
     // the free-flight and hand-over queues hold at most one record per input superphoton and launch, and are sized
     // for a whole tracker input: an overflow there is a logic error, reported, never a silent loss
+    // the cascade sends the leavers of ALL remaining generations to the free-flight queue in one launch: if that
+    // overflows, the caller restores its snapshot and redoes the batch without the cascade
+    if (cascaded && (h_counts[67] & ~2) == 0 && h_counts[64] <= parkA.capacity && h_counts[65] <= parkB.capacity &&
+        ((h_counts[67] & 2) || h_counts[2] > esc.capacity)) {
+      ctx->cascade_overflowed = true;
+      *max_queue = qcap + 1;
+      return GM_OK;
+    }
     if (h_counts[67] != 0 || h_counts[64] > parkA.capacity || h_counts[65] > parkB.capacity || h_counts[2] > esc.capacity)
       return fail(ctx, GM_ERR_OVERFLOW, "internal queue overflow (flags %d; free-flight %d/%d, hand-over %d, %d/%d records)",
                   h_counts[67], h_counts[2], esc.capacity, h_counts[64], h_counts[65], parkA.capacity);
@@ -556,6 +594,7 @@ static int run_range(gm_ctx* ctx, int64_t first_id, int64_t n_ids, Tally tally, 
     if (mq > ctx->queue_records) {
       CK(cudaMemcpyAsync(tally.A, ctx->tally_snap.A, (size_t)nb * 4 * sizeof(double), cudaMemcpyDeviceToDevice, st));
       CK(cudaMemcpyAsync(stats, ctx->d_stats_snap, sizeof(DevStats), cudaMemcpyDeviceToDevice, st));
+      if (ctx->cascade_overflowed) { ctx->cascade_overflowed = false; ctx->cascade_skip = true; continue; }   // same batch, no cascade
       if (nthis <= 256)
         return fail(ctx, GM_ERR_OVERFLOW, "scattered-superphoton queue (%lld records) overflows with a batch of %lld primaries; "
                     "raise it with gm_set_batch or lower the bias", ctx->queue_records, nthis);
@@ -566,6 +605,7 @@ static int run_range(gm_ctx* ctx, int64_t first_id, int64_t n_ids, Tally tally, 
       continue;
     }
     done += nthis;
+    ctx->cascade_skip = false;
   }
   return GM_OK;
 }
@@ -761,6 +801,11 @@ int gm_trace(gm_ctx* ctx, const int64_t* ids, int n, gm_trace_rec* out) {
     int mq = 0;
     TraceBuf tb{d_rec + done};
     rc = run_batch(ctx, 0, (int)nthis, d_ids, tb, true, scratch, d_st, 0, &mq);
+    if (rc == GM_OK && mq > ctx->queue_records && ctx->cascade_overflowed) {
+      ctx->cascade_overflowed = false; ctx->cascade_skip = true;
+      continue;                                          // the same chunk again, without the cascade
+    }
+    ctx->cascade_skip = false;
     if (rc == GM_OK && mq > ctx->queue_records) {
       if (nthis <= 16) rc = fail(ctx, GM_ERR_OVERFLOW, "gm_trace: scattered-superphoton queue overflow");
       else { chunk = nthis / 2; continue; }

@@ -50,6 +50,9 @@ cudaError_t launch_track(const DevParams& P, int phase, const Photon* in, const 
                          DevStats* stats, TraceBuf trace, int* overflow, int n_sm, cudaStream_t st);
 // opt-in for > 48 KB of dynamic shared memory of every track_kernel instance, on the CURRENT device
 cudaError_t track_kernel_optin();
+// records of the per-warp event stacks a PHASE_CASCADE launch needs (all warps of its grid) and records per warp
+long long track_wstack_records(int n_sm);
+int track_wstack_per_warp();
 // free flight of the leavers to r_max (record) ; a superphoton that re-enters the grid is appended to `ret`
 // `overflow`: sticky device flag word; a consumer kernel ORs 1 (tracker input) / 2 (free-flight queue) into it when
 // the queue it reads was filled past its capacity

@@ -206,6 +206,16 @@ __global__ void __launch_bounds__(128, GM_EMIT_MINBLOCKS) emit_kernel(const DevP
 // A history is a pure function of its record (counter-based RNG), so the passes change no result.
 // =====================================================================================================
 constexpr int PHASE_MIXED = 0, PHASE_HOT = 1, PHASE_COLD = 2;
+// PHASE_CASCADE: the mixed pass for the small late generations of a batch.  A generation of a few thousand superphotons
+// costs a launch that lasts as long as its histories (the machine is almost empty), and nsc_max of them run one after
+// the other.  Here a warp keeps the scattering events of its own lanes on a private stack (global memory, `park.buf`
+// + warp * `park.capacity` records; the count in shared memory), turns them into superphotons itself when lanes
+// fall free (cascade_convert = the Compton kernel's event code, out of line) and tracks them at once: all remaining
+// generations in ONE launch, no exchange between warps.  A full stack sends the event to the `out` queue as usual.
+constexpr int PHASE_CASCADE = 3;
+constexpr int WSTACK_RECORDS = 128;                 // per warp
+template <bool KERR, bool THREED>
+__device__ bool cascade_convert(const DevParams& P, Photon* ph, DevStats* stats, TraceBuf trace);
 #ifndef GM_SMALL_PASS
 #define GM_SMALL_PASS 262144
 #endif
@@ -473,6 +483,9 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
   for (int m = 0; m < 4; m++) { L.x[m] = 0.0; L.k[m] = 0.0; L.a[m] = 0.0; }
   __shared__ uint4 s_cb[TRACK_WARPS][32];                 // cold pass: the cell bounds of each lane's end point
   uint4* const stage_cb = s_cb[wid];
+  __shared__ int s_wstk[TRACK_WARPS];                     // cascade: records on this warp's private event stack
+  if (PHASE == PHASE_CASCADE && lane == 0) s_wstk[wid] = 0;
+  Photon* const wstack = PHASE == PHASE_CASCADE ? park.buf + (size_t)(blockIdx.x * TRACK_WARPS + wid) * park.capacity : nullptr;
   bool have = false;
   int ncold = 0;                        // PHASE_HOT: consecutive committed cold steps of this lane
   int mode = 0;                         // 0 normal step, 1 partial push to a scattering event, 2 redo full step
@@ -487,7 +500,7 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
   for (;;) {
     __syncwarp();
     // ---- refill the stopped lanes of this warp together ----
-    const unsigned need = __ballot_sync(0xffffffffu, !have);
+    unsigned need = __ballot_sync(0xffffffffu, !have);
     // Stragglers: once this warp's input is exhausted and only `carry_lanes` or fewer of its lanes still fly, their
     // records go to the free-flight queue marked FLAG_CARRY; escape_kernel hands them unchanged to the next
     // generation's launch, where they continue inside full warps.  The launch then ends with its bulk instead of
@@ -502,6 +515,21 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
         have = false;
       }
       break;
+    }
+    if (PHASE == PHASE_CASCADE && need) {
+      // events of this warp's own lanes first: each free lane pops one, makes it a superphoton and tracks it
+      const int ns = *(volatile int*)&s_wstk[wid];
+      if (ns > 0) {
+        const int take = min(__popc(need), ns), rank = __popc(need & lt_mask);
+        if (!have && rank < take) {
+          Photon ph = wstack[ns - 1 - rank];
+          if (cascade_convert<KERR, THREED>(P, &ph, stats, trace)) { lane_load(L, &ph); have = true; mode = 0; ncold = 0; }
+        }
+        __syncwarp();
+        if (lane == 0) s_wstk[wid] = ns - take;
+        __syncwarp();
+        need = __ballot_sync(0xffffffffu, !have);
+      }
     }
     if (need) {
       if (st_next == st_avail && !exhausted) {
@@ -529,7 +557,7 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
         }
         st_next += min(__popc(need), left);
         __syncwarp();
-      } else if (exhausted && need == 0xffffffffu) {
+      } else if (exhausted && need == 0xffffffffu && (PHASE != PHASE_CASCADE || *(volatile int*)&s_wstk[wid] == 0)) {
         break;
       }
     }
@@ -645,9 +673,16 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
 #pragma unroll
       for (int m = 0; m < 4; m++) { L.x[m] = x1[m]; L.k[m] = k1[m]; L.a[m] = a1[m]; }
       const double wc = wev / ev_b;                          // child weight w/b
-      const int slot = atomicAdd(out.count, 1);
-      if (slot < out.capacity) {
-        Photon* c = out.buf + slot;
+      Photon* c = nullptr;
+      if (PHASE == PHASE_CASCADE) {
+        const int sl = atomicAdd(&s_wstk[wid], 1);
+        if (sl < park.capacity) c = wstack + sl; else atomicSub(&s_wstk[wid], 1);
+      }
+      if (!c) {
+        const int slot = atomicAdd(out.count, 1);
+        if (slot < out.capacity) c = out.buf + slot;
+      }
+      if (c) {
         double2* c2 = reinterpret_cast<double2*>(c);
         c2[0] = make_double2(L.x[0], L.x[1]); c2[1] = make_double2(L.x[2], L.x[3]);
         c2[2] = make_double2(L.k[0], L.k[1]); c2[3] = make_double2(L.k[2], L.k[3]);
@@ -1057,6 +1092,40 @@ __device__ inline bool compton_event(const DevParams& P, const Geom& G, const Pl
   return ok;
 }
 
+// the parent state at a scattering event (a record of the tracker's `out` queue) -> the scattered superphoton, in place
+template <bool KERR, bool THREED>
+__device__ __forceinline__ bool compton_convert(const DevParams& P, Photon& ph) {
+  Geom G; DGeom D;
+  geom_at<KERR, true>(P, ph.x[1], ph.x[2], G, &D);
+  Plasma S;
+  bool inplasma = plasma_at<THREED>(P, ph.x, G, S);    // true by construction (tested by the tracker)
+  double kout[4];
+  if (!(inplasma && compton_event(P, G, S, ph.k, ph.id0, ph.id1, ph.id2, ph.jscat, kout))) return false;
+  uint32_t o[4];
+  philox4x32_10(ph.id0, ph.id1, ph.id2, ph.jscat, P.seed_lo ^ TAG_SPAWN, P.seed_hi, o);
+  ph.id0 = o[0]; ph.id1 = o[1]; ph.id2 = o[2];
+  for (int m = 0; m < 4; m++) ph.k[m] = kout[m];
+  accel<KERR>(G, D, ph.k, ph.a);
+  ph.nsc += 1; ph.nstep = 0; ph.jscat = 0; ph.flags = 0;
+  opacities(P, ph.k, G, S, ph.nsc, P.scattering_on != 0 && ph.nsc < P.nsc_max, ph.nua_a, ph.nua_s, ph.bias);
+  return true;
+}
+// the same for one record of a cascade warp's private stack, with the Compton kernel's bookkeeping (out of line: the
+// event code is as large as the tracker's loop)
+template <bool KERR, bool THREED>
+__device__ __noinline__ bool cascade_convert(const DevParams& P, Photon* ph, DevStats* stats, TraceBuf trace) {
+  if (compton_convert<KERR, THREED>(P, *ph)) {
+    atomicAdd(&stats->n[SN_SPAWNED], 1ull);
+    atomicAdd(&stats->s[SS_SPAWNED], ph->w);
+    atomicAdd(&stats->gen[(ph->nsc - 1) & 63], 1ull);
+    if (trace.rec && ph->root >= 0) atomicAdd((unsigned long long*)&trace.rec[ph->root].fam_nspawn, 1ull);
+    return true;
+  }
+  atomicAdd(&stats->n[SN_BADSCAT], 1ull);
+  atomicAdd(&stats->s[SS_BAD], ph->w);
+  return false;
+}
+
 template <bool KERR, bool THREED>
 // The event body is a chain of rejection loops (Maxwell-Juttner, Klein-Nishina): divergent and latency-bound, so
 // it wants warps, not registers.  Measured per cfg2 step: 254 registers (8 warps/SM) 17.8 ms, 128 (16) 13.2,
@@ -1070,20 +1139,8 @@ __global__ void __launch_bounds__(128, GM_COMPTON_MINBLOCKS) compton_kernel(cons
   double s_bad = 0.0, s_spawn = 0.0;
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
     Photon ph = q.buf[i];
-    Geom G; DGeom D;
-    geom_at<KERR, true>(P, ph.x[1], ph.x[2], G, &D);
-    Plasma S;
-    bool inplasma = plasma_at<THREED>(P, ph.x, G, S);    // true by construction (tested by the tracker)
-    double kout[4];
-    bool ok = inplasma && compton_event(P, G, S, ph.k, ph.id0, ph.id1, ph.id2, ph.jscat, kout);
+    const bool ok = compton_convert<KERR, THREED>(P, ph);
     if (ok) {
-      uint32_t o[4];
-      philox4x32_10(ph.id0, ph.id1, ph.id2, ph.jscat, P.seed_lo ^ TAG_SPAWN, P.seed_hi, o);
-      ph.id0 = o[0]; ph.id1 = o[1]; ph.id2 = o[2];
-      for (int m = 0; m < 4; m++) ph.k[m] = kout[m];
-      accel<KERR>(G, D, ph.k, ph.a);
-      ph.nsc += 1; ph.nstep = 0; ph.jscat = 0; ph.flags = 0;
-      opacities(P, ph.k, G, S, ph.nsc, P.scattering_on != 0 && ph.nsc < P.nsc_max, ph.nua_a, ph.nua_s, ph.bias);
       c_spawn++; s_spawn += ph.w;
       {                                                    // per-generation count (bias tuning, G32): one atomic per warp and generation
         const int g = ph.nsc - 1;
@@ -1251,9 +1308,13 @@ cudaError_t track_kernel_optin() {
   GM_OPTIN(true, true, PHASE_MIXED); GM_OPTIN(true, false, PHASE_MIXED); GM_OPTIN(false, true, PHASE_MIXED);
   GM_OPTIN(false, false, PHASE_MIXED); GM_OPTIN(true, true, PHASE_HOT); GM_OPTIN(true, false, PHASE_HOT);
   GM_OPTIN(true, true, PHASE_COLD); GM_OPTIN(true, false, PHASE_COLD);
+  GM_OPTIN(true, true, PHASE_CASCADE); GM_OPTIN(true, false, PHASE_CASCADE); GM_OPTIN(false, true, PHASE_CASCADE); GM_OPTIN(false, false, PHASE_CASCADE);
 #undef GM_OPTIN
   return e;
 }
+
+long long track_wstack_records(int n_sm) { return (long long)n_sm * GM_TRACK_MINBLOCKS * TRACK_WARPS * WSTACK_RECORDS; }
+int track_wstack_per_warp() { return WSTACK_RECORDS; }
 
 cudaError_t launch_track(const DevParams& P, int phase, const Photon* in, const int* in_count, int in_capacity,
                          int* work_counter, Queue out, Queue esc, Queue park, int k_cold, int carry_lanes, Tally tally,
@@ -1269,6 +1330,11 @@ cudaError_t launch_track(const DevParams& P, int phase, const Photon* in, const 
     else if (kerr) track_kernel<true, false, PHASE_MIXED><<<grid, TRACK_THREADS, smem, st>>>(GM_TRACK_ARGS);
     else if (td) track_kernel<false, true, PHASE_MIXED><<<grid, TRACK_THREADS, smem, st>>>(GM_TRACK_ARGS);
     else track_kernel<false, false, PHASE_MIXED><<<grid, TRACK_THREADS, smem, st>>>(GM_TRACK_ARGS);
+  } else if (phase == PHASE_CASCADE) {
+    if (kerr && td) track_kernel<true, true, PHASE_CASCADE><<<grid, TRACK_THREADS, smem, st>>>(GM_TRACK_ARGS);
+    else if (kerr) track_kernel<true, false, PHASE_CASCADE><<<grid, TRACK_THREADS, smem, st>>>(GM_TRACK_ARGS);
+    else if (td) track_kernel<false, true, PHASE_CASCADE><<<grid, TRACK_THREADS, smem, st>>>(GM_TRACK_ARGS);
+    else track_kernel<false, false, PHASE_CASCADE><<<grid, TRACK_THREADS, smem, st>>>(GM_TRACK_ARGS);
   } else if (!kerr) {
     return cudaErrorInvalidValue;        // phase passes are instantiated for the Kerr workloads only
   } else if (phase == PHASE_HOT) {

@@ -480,6 +480,42 @@ def test_straggler_carry_over_changes_no_history(gm, cfg, monkeypatch):
         assert np.array_equal(t0["w"], t1["w"]) and np.array_equal(t0["x"], t1["x"])
 
 
+@pytest.mark.parametrize("cfg", [2, 3, 4])
+def test_cascade_pass_changes_no_history(gm, cfg, monkeypatch):
+    """The small late generations of a batch are tracked in ONE launch in which every warp converts and tracks the
+    scattering events of its own lanes from a private stack (PHASE_CASCADE; threshold read from
+    GPUMONTY_B200_CASCADE at gm_create).  Never, the default, and "from the second generation on whatever its size"
+    (a stack of 128 records per warp then overflows into the ordinary queue, and on the small 3-D case the free-flight
+    queue overflows too, which makes the driver redo the batch without the cascade: the fall-back paths) must give
+    identical histories, families and counters.  (Kerr workloads only: DESIGN.md section 6.)"""
+    p, prim = {2: lambda: wl.config2(Ns=1e5),
+               3: lambda: wl.config3(Ns=2e4, n1=48, n2=32, n3=32), 4: lambda: wl.config4(Ns=2e5)}[cfg]()
+    res = []
+    for casc in ("0", None, "2000000000"):
+        if casc is None:
+            monkeypatch.delenv("GPUMONTY_B200_CASCADE", raising=False)
+        else:
+            monkeypatch.setenv("GPUMONTY_B200_CASCADE", casc)
+        g = gm.GPUMonty(p)
+        g.set_grid(prim)
+        g.prepare()
+        g.run()
+        ids = np.arange(0, g.n_primaries, 7)
+        res.append((g.stats(), g.tally(), g.trace(ids)))
+    s0, (A0, Q0, W0, n0), t0 = res[0]
+    assert s0["n_spawned"] > 1000
+    for s1, (A1, Q1, W1, n1), t1 in res[1:]:
+        for k in s0:
+            if k.startswith("n_"):
+                assert s0[k] == s1[k], (k, s0[k], s1[k])
+            else:
+                assert s1[k] == pytest.approx(s0[k], rel=1e-11, abs=1e-300), k
+        assert np.array_equal(n0, n1) and np.allclose(A0, A1, rtol=1e-11, atol=0)
+        for f in ("fate", "nstep", "inu", "ith", "jscat", "fam_nspawn"):
+            assert np.array_equal(t0[f], t1[f]), f
+        assert np.array_equal(t0["w"], t1["w"]) and np.array_equal(t0["x"], t1["x"])
+
+
 @pytest.mark.parametrize("scattering", [False, True])
 def test_partial_cell_sphere_boundary(gm, scattering):
     """the sphere surface cuts a radial zone; densities scaled by the 5 x 5
