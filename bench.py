@@ -293,9 +293,13 @@ def main():
             rate = pr["tracked"] / max(pr["run_s"], 1e-6)
             n_sample = int(max(20000, rate * 15.0 / (pr["tracked"] / max(1, pr["n_sample"]))))
             r = oracle_sample(p, prim, n_sample)
+            r1 = oracle_sample(p, prim, max(2000, n_sample // (4 * max(1, r["cores"]))), threads=1)   # ~4 s on one thread
             out["cpu_baseline"] = {"value": r["tracked"] / r["run_s"], "unit": UNIT, "cores": r["cores"], "kind": "oracle",
                                    "sample": f"first {r['n_sample']} primaries + descendants ({r['tracked']} superphotons, "
-                                             f"{r['run_s']:.1f} s, oracle prepare {r['prepare_s']:.1f} s not counted)"}
+                                             f"{r['run_s']:.1f} s, oracle prepare {r['prepare_s']:.1f} s not counted)",
+                                   "one_thread": {"value": r1["tracked"] / r1["run_s"], "unit": UNIT, "cores": r1["cores"],
+                                                  "sample": f"first {r1['n_sample']} primaries + descendants "
+                                                            f"({r1['tracked']} superphotons, {r1['run_s']:.1f} s)"}}
         g.close()
         del dev_grid, host_grid
         torch.cuda.empty_cache()
