@@ -313,7 +313,7 @@ def test_scan_ragged_tail_and_empty_zones(gm):
 # ---------------------------------------------------------------------------------------------------
 # S6-S12: histories and spectra
 # ---------------------------------------------------------------------------------------------------
-def _compare_traces(o, g, ids, fork_budget, label=None):
+def _compare_traces(o, g, ids, fork_budget, label=None, x_tol=1e-7):
     """Same-stream histories one by one.  A history "forks" when a uniform falls within rounding of a threshold
     (or libdevice and glibc differ in the last ulp of a transcendental): every integer of its final state is
     compared, the forks are counted, printed and (on the GPU box) appended to gpurun_out/fork_rates.md; the budget
@@ -336,7 +336,11 @@ def _compare_traces(o, g, ids, fork_budget, label=None):
     assert np.max(_relerr(tg["w"][ok], to["w"][ok])) < 1e-7
     rec = ok[to["fate"][ok] == 1]
     assert np.max(_relerr(tg["E_inf"][rec], to["E_inf"][rec])) < 1e-7
-    assert np.max(np.abs(tg["x"][ok] - to["x"][ok])) < 1e-7
+    dx = np.max(np.abs(tg["x"][ok] - to["x"][ok]), axis=1)
+    if x_tol != 1e-7:
+        print("largest final-position difference %.2e (history of %d steps); %d of %d above 1e-7"
+              % (dx.max(), tg["nstep"][ok][np.argmax(dx)], np.count_nonzero(dx >= 1e-7), len(ok)))
+    assert dx.max() < x_tol
     # family sums: only compare where the spawn counts agree (a fork inside a child changes them)
     assert len(fsame) >= (1 - 10 * fork_budget) * len(ok) - 1
     assert np.max(_relerr(tg["fam_wE"][fsame], fam_wE[fsame], floor=1e-300)) < 1e-6
@@ -682,21 +686,24 @@ def _full_size_checks(gm, p, prim, n_sample, seed):
            sg["sum_w_outofrange"] + sg["sum_w_maxstep"] + sg["sum_w_absorbed"] + sg["sum_w_bad"])
     assert out == pytest.approx(sg["sum_w_emit"], rel=1e-9)
     ids = np.sort(np.random.default_rng(seed).choice(g.n_primaries, n_sample, replace=False))
-    _compare_traces(o, g, ids, fork_budget=2e-4)
+    # (20,000 histories: rounding-order differences of 1e-16 per step are amplified along the longest ones -- thousands of
+    # small steps next to the polar axis -- to just above the 1e-7 that the smaller samples never reach; every integer of
+    # those histories is still equal.  DESIGN.md section 3.)
+    _compare_traces(o, g, ids, fork_budget=2e-4, x_tol=1e-6)
     return sg
 
 
 def test_full_size_config2(gm):
     """BASELINE configs[2] as bench.py runs it: 256x256 Kerr torus, N_s = 1e7 (3.6e6 primaries, 2.5e7 scattered)."""
     p, prim = wl.config2()
-    sg = _full_size_checks(gm, p, prim, 3000, 21)
+    sg = _full_size_checks(gm, p, prim, 20000, 21)
     assert sg["n_spawned"] > 5 * sg["n_primary"]
 
 
 def test_full_size_config1(gm):
     """BASELINE configs[1] at N_s = 1e6."""
     p, prim = wl.config1()
-    _full_size_checks(gm, p, prim, 3000, 22)
+    _full_size_checks(gm, p, prim, 20000, 22)
 
 
 def test_batching_and_queue_overflow_recovery(gm):
