@@ -140,7 +140,8 @@ void gm_destroy(gm_ctx* ctx);
 /* (Re)build the parameter-free device tables K2, F and (if scattering_on) sigma_h on `cuda_stream`
  * (PAPER.md:166, 188).  gm_create calls it once; a benchmark may call it per step. */
 int gm_build_tables(gm_ctx* ctx, void* cuda_stream);
-/* Message of the last failing call on ctx (or of the last failing gm_create when ctx == NULL). */
+/* Message of the last failing call on ctx (ctx == NULL: of the last failing context-free call, i.e. gm_create,
+ * gm_fp64_peak or gm_scan_counts_static). */
 const char* gm_last_error(const gm_ctx* ctx);
 
 /* Fluid grid prim[n1][n2][n3][8] = rho, u, u~1, u~2, u~3, B1, B2, B3 in code units, zone-major fp64
@@ -155,6 +156,37 @@ int gm_set_grid(gm_ctx* ctx, const double* prim, int on_device, size_t n_bytes, 
 int gm_prepare(gm_ctx* ctx, void* cuda_stream, int64_t* n_primaries_out);
 
 int gm_get_zone_counts(gm_ctx* ctx, int32_t* counts /* [n1*n2*n3] */);
+/* The exclusive prefix sum gm_prepare formed from those counts: offsets[z] = id of the first primary of zone z,
+ * offsets[n1*n2*n3] = number of primaries.  `offsets` is a HOST array of n1*n2*n3 + 1 values. */
+int gm_get_zone_offsets(gm_ctx* ctx, int64_t* offsets /* [n1*n2*n3 + 1] */);
+
+/* The same prefix sum (zone counts -> which zone a primary id belongs to) as a
+ * stand-alone call that allocates nothing -- no cudaMalloc / cudaFree, no allocating library routine, no context.
+ *
+ * Who needs it: code that is not allowed to ask the CUDA allocator for memory at the point where it wants the scan.
+ * Typical cases are a module hosted by an application whose own pool has reserved the device and forbids outside
+ * allocations, and a latency-bound loop that cannot afford cudaMalloc's implicit device-wide synchronisation.  Such a
+ * caller cannot use gm_create / gm_prepare (they allocate); it brings its own buffers and calls this instead.
+ *
+ *   d_counts   DEVICE, n_zones int32 values >= 0 (the caller's; read only)
+ *   d_offsets  DEVICE, n_zones + 1 int64 values (the caller's): d_offsets[z] = sum of d_counts[0..z), the last
+ *              one the total.  Bit-identical to what gm_prepare computes (gm_get_zone_offsets).
+ *   n_zones    0 .. GM_SCAN_STATIC_MAX_ZONES.  Anything larger is refused with GM_ERR_PARAM and a message naming the
+ *              limit; nothing is launched.  The limit exists because the partial sums between the phases of the scan
+ *              (one int64 per 1024 zones) sit in a fixed 32 KiB array compiled into the library.  Every GPU that loads
+ *              the library carries that array until the process ends, used or not; it cannot be resized or released.
+ *
+ * The first call on each device looks up the array's device address (cudaGetSymbolAddress, with that device current)
+ * and makes CUDA load the kernels; make that first call outside any stream capture.  Later calls only enqueue three
+ * small kernels on `cuda_stream` and return without synchronising.
+ * All calls on one device share the one array.  It keeps whatever the previous call left there; that is harmless
+ * (each call overwrites every element it later reads), but two calls that can run on the GPU at the same time --
+ * different streams, or different host threads on different streams -- overwrite each other's partial sums and return
+ * garbage.  Keep calls on one stream, or order them with events.
+ * Errors: GM_ERR_PARAM (NULL pointer, n_zones out of range), GM_ERR_CUDA (no device, look-up or launch failed); the text
+ * is available from gm_last_error(NULL). */
+#define GM_SCAN_STATIC_MAX_ZONES 4194304 /* 4096 tiles of 1024 zones; cfg3's 192x128x128 grid has 3,145,728 */
+int gm_scan_counts_static(const int32_t* d_counts, int64_t n_zones, int64_t* d_offsets, void* cuda_stream);
 /* Copy a table to `out`; n must equal the table's length (else GM_ERR_PARAM). */
 int gm_get_table(gm_ctx* ctx, int which, double* out, size_t n);
 

@@ -25,7 +25,8 @@ FATE_ALIVE, FATE_RECORDED, FATE_HORIZON, FATE_ROULETTE, FATE_MAXSTEP, FATE_OUTOF
 EXPORTS = ["gm_create", "gm_destroy", "gm_last_error", "gm_set_grid", "gm_prepare", "gm_get_zone_counts",
            "gm_get_table", "gm_run", "gm_set_batch", "gm_set_phase_passes", "gm_get_spectrum", "gm_get_tally", "gm_get_stats",
            "gm_reset_tally", "gm_emit", "gm_trace", "gm_eval", "gm_fp64_peak", "gm_build_tables", "gm_timing", "gm_spectrum_device",
-           "gm_get_bias_table", "gm_set_bias_table"]
+           "gm_get_bias_table", "gm_set_bias_table", "gm_get_zone_offsets", "gm_scan_counts_static"]
+SCAN_STATIC_MAX_ZONES = 4194304  # GM_SCAN_STATIC_MAX_ZONES
 
 
 class GmParams(C.Structure):
@@ -112,6 +113,8 @@ def load_library(build_if_missing: bool = True) -> C.CDLL:
     L.gm_timing.argtypes = [vp, C.c_int, vp, vp]
     L.gm_get_bias_table.argtypes = [vp, vp, vp, C.POINTER(C.c_int)]
     L.gm_set_bias_table.argtypes = [vp, vp]
+    L.gm_get_zone_offsets.argtypes = [vp, vp]
+    L.gm_scan_counts_static.argtypes = [vp, C.c_int64, vp, vp]
     L.gm_abi_sizes.restype = None
     _lib = L
     return L
@@ -157,6 +160,24 @@ def fp64_peak():
     if rc:
         raise GmError(rc, L.gm_last_error(None).decode())
     return f.value, c.value
+
+
+def scan_counts_static(counts, offsets, n_zones=None, stream=None):
+    """gm_scan_counts_static: exclusive prefix sum of `counts` (CUDA int32 tensor) into `offsets` (CUDA int64 tensor,
+    one element longer), for callers that may not allocate device memory: no context, no cudaMalloc; the scan's
+    partial sums go to a fixed array inside the library, hence n_zones <= SCAN_STATIC_MAX_ZONES and no two calls in
+    flight at once on a device.  Both tensors are the caller's; nothing is returned and nothing is synchronised.
+    `n_zones` defaults to counts.numel() (passing it explicitly exists for the size-limit test)."""
+    import torch
+    L = load_library()
+    assert counts.is_cuda and offsets.is_cuda and counts.dtype == torch.int32 and offsets.dtype == torch.int64
+    assert counts.is_contiguous() and offsets.is_contiguous()
+    n = counts.numel() if n_zones is None else int(n_zones)
+    if n_zones is None:
+        assert offsets.numel() == n + 1
+    rc = L.gm_scan_counts_static(C.c_void_p(counts.data_ptr()), n, C.c_void_p(offsets.data_ptr()), _stream_ptr(stream))
+    if rc:
+        raise GmError(rc, L.gm_last_error(None).decode())
 
 
 class GPUMonty:
@@ -245,6 +266,11 @@ class GPUMonty:
     def zone_counts(self):
         o = np.zeros(self.nz, dtype=np.int32)
         self._ck(self.L.gm_get_zone_counts(self.h, _np_ptr(o)))
+        return o
+
+    def zone_offsets(self):
+        o = np.zeros(self.nz + 1, dtype=np.int64)
+        self._ck(self.L.gm_get_zone_offsets(self.h, _np_ptr(o)))
         return o
 
     def table(self, which):

@@ -176,6 +176,10 @@ static void fill_dev_params(gm_ctx* c) {
   P.prim = c->d_prim; P.lnK2 = c->d_lnK2; P.lnF = c->d_lnF; P.lnSigH = c->d_lnSigH; P.lnw = c->d_lnw;
 }
 
+namespace gm {
+void note_global_error(const char* msg) { g_create_err = msg ? msg : ""; }
+}  // namespace gm
+
 extern "C" {
 
 static int tune_bias(gm_ctx* ctx, cudaStream_t st);
@@ -338,6 +342,14 @@ int gm_get_zone_counts(gm_ctx* ctx, int32_t* counts) {
   if (!ctx || !counts) return GM_ERR_PARAM;
   if (!ctx->prepared) return fail(ctx, GM_ERR_STATE, "not prepared");
   CK(cudaMemcpy(counts, ctx->Z.n, ctx->nz * sizeof(int32_t), cudaMemcpyDeviceToHost));
+  return GM_OK;
+}
+
+int gm_get_zone_offsets(gm_ctx* ctx, int64_t* offsets) {
+  if (!ctx || !offsets) return GM_ERR_PARAM;
+  if (!ctx->prepared) return fail(ctx, GM_ERR_STATE, "not prepared");
+  static_assert(sizeof(long long) == sizeof(int64_t), "offset type");
+  CK(cudaMemcpy(offsets, ctx->Z.offset, (ctx->nz + 1) * sizeof(long long), cudaMemcpyDeviceToHost));
   return GM_OK;
 }
 

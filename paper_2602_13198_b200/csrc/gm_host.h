@@ -4,6 +4,9 @@
 
 namespace gm {
 
+// ---- gm_api.cu: text for gm_last_error(NULL), for entry points that have no context ------------------------
+void note_global_error(const char* msg);
+
 // ---- gm_tables.cu: parameter-free tables, weights, zone counts, prefix sum ----------------------
 // device arrays of length NK2+1, NF+1, (NSE+1)*(NST+1)
 cudaError_t build_K2_table(double* d_lnK2, cudaStream_t st);

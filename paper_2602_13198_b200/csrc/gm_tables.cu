@@ -12,6 +12,8 @@
 #include "gm_host.h"
 #include "gm_physics.cuh"
 #include <cmath>
+#include <cstdio>
+#include <mutex>
 #include <vector>
 
 namespace gm {
@@ -414,3 +416,81 @@ cudaError_t launch_prepare(const DevParams& P, const ZoneArrays& Z, double* d_ln
 }
 
 }  // namespace gm
+
+// ------------------------------------------------------------------------------------------------
+// gm_scan_counts_static: the S4 prefix sum for callers that must not allocate (include/gpumonty_b200.h).
+//
+// The three-phase scan above needs one partial sum per 1024-zone tile between its phases.  gm_prepare keeps those in
+// a cudaMalloc'ed buffer of the context.  This entry point is for code that has no context and may not call
+// cudaMalloc at all -- a plugin running inside a host application whose memory pool owns the whole device, a step
+// replayed inside someone else's captured region, a real-time loop that must not hit the allocator's device-wide
+// lock -- so its tile sums live in the file-scope array below, which is part of the library's image: every GPU that
+// loads the library holds these 32 KiB from load to exit, whether or not the entry point is ever called.
+//
+// `g_scan_static_tiles` as written in HOST code is only the host-side handle of that symbol, not an address the GPU
+// can use (a kernel handed it would fault, or on a system where the GPU can reach host memory quietly scribble over
+// whatever host data sits there).  The device address is looked up with cudaGetSymbolAddress, once per device, with
+// that device current, and that pointer is what the kernels get.
+constexpr long GM_SCAN_STATIC_TILES = GM_SCAN_STATIC_MAX_ZONES / gm::SCAN_TILE;
+static_assert(GM_SCAN_STATIC_TILES * gm::SCAN_TILE == GM_SCAN_STATIC_MAX_ZONES, "maximum must be whole tiles");
+static __device__ __align__(256) long long g_scan_static_tiles[GM_SCAN_STATIC_TILES];
+
+namespace {
+constexpr int SCAN_STATIC_MAX_DEVICES = 64;
+long long* s_scan_static_addr[SCAN_STATIC_MAX_DEVICES];   // device address of the array, per device ordinal (0: not looked up yet)
+std::mutex s_scan_static_mutex;
+}  // namespace
+
+extern "C" int gm_scan_counts_static(const int32_t* d_counts, int64_t n_zones, int64_t* d_offsets, void* cuda_stream) {
+  char msg[256];
+  if (!d_counts || !d_offsets) { gm::note_global_error("gm_scan_counts_static: d_counts / d_offsets is NULL"); return GM_ERR_PARAM; }
+  if (n_zones < 0 || n_zones > (int64_t)GM_SCAN_STATIC_MAX_ZONES) {
+    snprintf(msg, sizeof(msg), "gm_scan_counts_static: n_zones = %lld is outside [0, %lld] (GM_SCAN_STATIC_MAX_ZONES: the built-in "
+             "scratch holds one partial sum per 1024 zones and cannot grow)", (long long)n_zones, (long long)GM_SCAN_STATIC_MAX_ZONES);
+    gm::note_global_error(msg);
+    return GM_ERR_PARAM;
+  }
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) {
+    snprintf(msg, sizeof(msg), "gm_scan_counts_static: no CUDA device (%s): this library has no CPU path", cudaGetErrorString(e));
+    gm::note_global_error(msg);
+    return GM_ERR_CUDA;
+  }
+  if (dev < 0 || dev >= SCAN_STATIC_MAX_DEVICES) {
+    snprintf(msg, sizeof(msg), "gm_scan_counts_static: device ordinal %d not supported (< %d)", dev, SCAN_STATIC_MAX_DEVICES);
+    gm::note_global_error(msg);
+    return GM_ERR_PARAM;
+  }
+  long long* tiles = nullptr;
+  {  // set-up, first call on this device only: ask the runtime where this device keeps its copy of the array
+    std::lock_guard<std::mutex> lock(s_scan_static_mutex);
+    if (!s_scan_static_addr[dev]) {
+      void* p = nullptr;
+      e = cudaGetSymbolAddress(&p, g_scan_static_tiles);
+      if (e != cudaSuccess || !p) {
+        snprintf(msg, sizeof(msg), "gm_scan_counts_static: cudaGetSymbolAddress(scratch) on device %d: %s", dev, cudaGetErrorString(e));
+        gm::note_global_error(msg);
+        return GM_ERR_CUDA;
+      }
+      s_scan_static_addr[dev] = (long long*)p;
+    }
+    tiles = s_scan_static_addr[dev];
+  }
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const long nz = (long)n_zones;
+  const int ntile = (int)((nz + gm::SCAN_TILE - 1) / gm::SCAN_TILE);
+  long long* off = reinterpret_cast<long long*>(d_offsets);
+  // Nothing in the array has to start at zero: phase 1 writes tiles[0 .. ntile), phases 2 and 3 read only those, so
+  // what an earlier call (of another size) left beyond ntile is never looked at.
+  if (ntile > 0) gm::scan_tile_sum_kernel<<<ntile, 256, 0, st>>>(d_counts, nz, tiles);
+  gm::scan_blocksum_kernel<<<1, 32, 0, st>>>(tiles, ntile, off, nz);      // also writes d_offsets[n_zones] = total
+  if (ntile > 0) gm::scan_tile_kernel<<<ntile, 256, 0, st>>>(d_counts, nz, tiles, off);
+  e = cudaGetLastError();
+  if (e != cudaSuccess) {
+    snprintf(msg, sizeof(msg), "gm_scan_counts_static: launch failed: %s", cudaGetErrorString(e));
+    gm::note_global_error(msg);
+    return GM_ERR_CUDA;
+  }
+  return GM_OK;
+}
