@@ -154,6 +154,14 @@ void orc_stream(uint64_t seed, uint32_t tag, uint32_t c0, uint32_t c1, uint32_t 
   Stream s(seed, tag, c0, c1, c2);
   for (int i = 0; i < n; i++) out[i] = s.next();
 }
+// spawn keying (G11): ids of the children of n (parent id, event ordinal j) pairs; parents[n][3], j[n] -> out[n][3]
+void orc_child_ids(uint64_t seed, const uint32_t* parents, const uint32_t* j, int64_t n, uint32_t* out) {
+  for (int64_t i = 0; i < n; i++) {
+    PhotonId par = {parents[3 * i], parents[3 * i + 1], parents[3 * i + 2]};
+    PhotonId c = child_id(seed, par, j[i]);
+    out[3 * i] = c.i0; out[3 * i + 1] = c.i1; out[3 * i + 2] = c.i2;
+  }
+}
 double orc_K2_direct(double th) { return K2_direct(th); }
 double orc_F_direct(double K) { return F_direct(K); }
 double orc_sigma_kn(double e) { return sigma_kn_over_T(e); }

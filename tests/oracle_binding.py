@@ -111,6 +111,7 @@ class OracleLib:
         L.orc_philox.argtypes = [C.c_void_p] * 3
         L.orc_uniform_pair.argtypes = [C.c_uint64] + [C.c_uint32] * 5 + [C.c_void_p]
         L.orc_stream.argtypes = [C.c_uint64] + [C.c_uint32] * 4 + [C.c_int, C.c_void_p]
+        L.orc_child_ids.argtypes = [C.c_uint64, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p]
         for f in ("orc_gcov", "orc_gcon", "orc_dgcov", "orc_conn"):
             getattr(L, f).argtypes = [C.POINTER(Params), C.c_void_p, C.c_void_p]
         L.orc_gdet.restype = C.c_double
@@ -139,6 +140,15 @@ class OracleLib:
     def stream(self, seed, tag, c0, c1, c2, n):
         o = np.zeros(n)
         self.L.orc_stream(seed, tag, c0, c1, c2, n, _p(o))
+        return o
+
+    def child_ids(self, seed, parents, j):
+        """ids [n][3] of the scattered superphotons spawned by event j[n] of parents[n][3] (G11)"""
+        par = np.ascontiguousarray(parents, dtype=np.uint32).reshape(-1, 3)
+        jj = np.ascontiguousarray(j, dtype=np.uint32)
+        assert len(jj) == len(par)
+        o = np.zeros_like(par)
+        self.L.orc_child_ids(seed, _p(par), _p(jj), len(jj), _p(o))
         return o
 
     def table(self, which):
