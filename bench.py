@@ -51,9 +51,24 @@ TRAFFIC_BYTES_PER_LAUNCH = {2: 2.897e9 + 2.832e9}
 TRAFFIC_SOURCE = {2: "profiles/r02_final.md (ncu --set full of this workload, cfg2 at N_s=1e7): hot tracker pass of the largest "
                      "scattering generation, 59 ms: reads 1.6e7 records of 160 B, writes as many hand-over / free-flight / "
                      "scattered records: DRAM traffic = algorithmic record bytes, the gather is served by L1/L2"}
-WORKLOAD_NAMES = {0: "cfg0 thin synchrotron sphere 32x16, Ns=1e5", 1: "cfg1 scattering sphere 32x16, Ns=1e6",
-                  2: "cfg2 Kerr FM torus 256x256, Ns=1e7", 3: "cfg3 3-D perturbed torus 192x128x128, Ns=1e7",
-                  4: "cfg4 Kerr torus x1e3 density (analog scattering), Ns=1e6"}
+# N_s at which FLOP_PER_STEP was counted (with the automatic pass schedule); at any other N_s, or with --phase-pairs /
+# --k-cold set, bounded and full steps mix differently and the constant is off by up to ~35 %: the line then says so
+FLOP_COUNTED_AT_NS = {0: 1e5, 1: 1e6, 2: 1e7, 3: 1e7, 4: 1e7}
+# algorithmic record bytes of the SAME launch TRAFFIC_BYTES_PER_LAUNCH was captured on (cfg2, hot pass of the largest
+# generation): 1.6e7 records of 160 B read, as many written
+TRAFFIC_LAUNCH_RECORD_BYTES = {2: 2 * 1.6e7 * 160.0}
+_WORKLOADS = {0: ("cfg0 thin synchrotron sphere 32x16", 1e5), 1: ("cfg1 scattering sphere 32x16", 1e6),
+              2: ("cfg2 Kerr FM torus 256x256", 1e7), 3: ("cfg3 3-D perturbed torus 192x128x128", 1e7),
+              4: ("cfg4 Kerr torus x1e3 density (analog scattering)", 1e6)}
+
+
+def workload_name(cfg: int, ns=None) -> str:
+    """Name of the workload with the N_s actually run (BASELINE.json's N_s of the config unless --ns overrides it)."""
+    name, default_ns = _WORKLOADS[cfg]
+    return f"{name}, Ns={(ns or default_ns):.0e}".replace("e+0", "e").replace("e+", "e")
+
+
+WORKLOAD_NAMES = {c: workload_name(c) for c in _WORKLOADS}
 
 
 def make_workload(cfg: int, ns: float | None, seed: int):
@@ -142,11 +157,12 @@ def run_reference(args, rank, world):
             times.append(r["run_s"] + r["prepare_s"]); tracked = r["tracked"]; cores = r["cores"]
     ms = 1e3 * float(np.mean(times))
     value = tracked / (ms * 1e-3)
-    sample = f"first {n_sample} primaries of {WORKLOAD_NAMES[args.config]} + all descendants per step (oracle prepare included)"
+    wname = workload_name(args.config, args.ns)
+    sample = f"first {n_sample} primaries of {wname} + all descendants per step (oracle prepare included)"
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": 0, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f64", "data": "synthetic", "config": {"workload": WORKLOAD_NAMES[args.config], "sample": sample},
+        "dtype": "f64", "data": "synthetic", "config": {"workload": wname, "sample": sample},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0}))
@@ -188,8 +204,10 @@ def main():
     peak_meas, _ = gm.fp64_peak()
     peak = peak_meas / 1e12
 
-    def measure(cfg: int, ns, steps: int, warmup: int, with_cpu_baseline: bool):
-        """All of the bench line for one workload: device-timed steps, e2e steps, roofline, clocks."""
+    def measure(cfg: int, ns, steps: int, warmup: int, with_cpu_baseline: bool, min_timed_s: float = 0.0):
+        """All of the bench line for one workload: device-timed steps, e2e steps, roofline, clocks.
+        min_timed_s > 0: as many timed steps as fill that time (small workloads: a step of a few ms ends before
+        the 200 ms clock sampler fires once; a sub-line without clock samples is no measurement)."""
         t_gen = time.perf_counter()
         p, prim = make_workload(cfg, ns, rank_seed(1, rank))
         gen_s = time.perf_counter() - t_gen
@@ -228,6 +246,9 @@ def main():
         for _ in range(warmup):
             step(False)
         torch.cuda.synchronize()
+        if min_timed_s > 0.0:
+            probe_ms = float(np.mean(timed(False, 2)))          # includes the L2 flush only as untimed work between steps
+            steps = int(min(500, max(steps, np.ceil(min_timed_s * 1e3 / max(probe_ms, 1e-3)))))
         g.timing(True)
         clocks = ClockSampler(local)
         clocks.start()
@@ -259,12 +280,14 @@ def main():
         # hand-over / free-flight / scattered record written once (160 B), 4 (2-D) or 8 (3-D) 64-byte zone lines
         # gathered per in-grid step (served by L1/L2 except on the 201 MB grid of cfg 3)
         lpl = max(1, n_track_launches // max(1, steps))
-        alg_bytes = ((tracked + st["n_spawned"]) * 160.0 + steps_track * (8 if p["n3"] > 1 else 4) * 64.0) / lpl
+        rec_bytes = (tracked + st["n_spawned"]) * 160.0 / lpl
+        gather_bytes = steps_track * (8 if p["n3"] > 1 else 4) * 64.0 / lpl
+        flop_valid = (args.phase_pairs < 0 and args.k_cold == 4 and (ns or _WORKLOADS[cfg][1]) == FLOP_COUNTED_AT_NS[cfg])
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warmup,
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic",
-            "config": {"workload": WORKLOAD_NAMES[cfg] + (f" (Ns overridden: {ns:g})" if ns else ""),
+            "config": {"workload": workload_name(cfg, ns),
                        "superphotons_per_step_per_gpu": tracked, "primaries": st["n_primary"], "spawned": st["n_spawned"],
                        "geodesic_steps": st["n_steps_total"], "geodesic_steps_free_flight": st["n_steps_free"],
                        "l2": "flushed between timed steps (256 MB write)", "host_generation_s": gen_s,
@@ -276,7 +299,14 @@ def main():
             "roofline": {"bound": "alu", "kernel": "track_kernel", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
                          "frac": achieved / peak, "traffic": TRAFFIC_BYTES_PER_LAUNCH.get(cfg),
                          "traffic_source": TRAFFIC_SOURCE.get(cfg),
-                         "algorithmic_bytes_per_launch": alg_bytes,
+                         # like for like with `traffic`: record bytes of the launch the capture was taken on, and their ratio
+                         "traffic_launch_algorithmic_record_bytes": TRAFFIC_LAUNCH_RECORD_BYTES.get(cfg),
+                         "traffic_over_algorithmic": (TRAFFIC_BYTES_PER_LAUNCH[cfg] / TRAFFIC_LAUNCH_RECORD_BYTES[cfg]
+                                                      if cfg in TRAFFIC_LAUNCH_RECORD_BYTES else None),
+                         # this run, averaged over ALL tracker launches of a step (not comparable with `traffic`):
+                         # record bytes (DRAM) and the zone lines the gathers ask for (served by L1/L2 on the 2-D grids)
+                         "avg_record_bytes_per_launch": rec_bytes, "avg_l2_gather_bytes_per_launch": gather_bytes,
+                         "flop_per_step_valid": bool(flop_valid),
                          "peak_source": "DFMA-chain microbenchmark run in this process (gm_fp64_peak); nominal 2*64*148*1.965 GHz = 37.2",
                          "flop_per_step": FLOP_PER_STEP[cfg]["track"], "track_ms_per_step": track_ms_per_step,
                          "flop_per_step_note": "algorithmic flop of THIS implementation (ncu-counted, profiles/r02_final.md); "
@@ -313,9 +343,10 @@ def main():
         for cfg, ns in ((3, None), (4, 1e7), (1, None), (0, None)):
             if cfg == args.config and not args.ns:
                 continue
-            r = measure(cfg, ns, 3, 3, False)
+            r = measure(cfg, ns, 3, 3, False, min_timed_s=1.2)
             others.append({"workload": r["config"]["workload"], "value": r["value"], "unit": UNIT,
-                           "ms_per_step": r["ms_per_step"], "e2e_value": r["e2e"]["value"],
+                           "ms_per_step": r["ms_per_step"], "steps": r["steps"], "e2e_value": r["e2e"]["value"],
+                           "flop_per_step_valid": r["roofline"]["flop_per_step_valid"],
                            "superphotons_per_step": r["config"]["superphotons_per_step_per_gpu"],
                            "tracker_frac_of_fp64_peak": r["roofline"]["frac"], "tracker_tflops": r["roofline"]["achieved"],
                            "track_share_of_step": r["roofline"]["track_share_of_step"],

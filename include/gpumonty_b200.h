@@ -31,7 +31,7 @@
 extern "C" {
 #endif
 
-#define GM_ABI_VERSION 2u
+#define GM_ABI_VERSION 3u
 
 enum {
   GM_OK = 0,
@@ -39,7 +39,8 @@ enum {
   GM_ERR_STATE = -2,    /* call order (e.g. gm_run before gm_prepare)    */
   GM_ERR_CUDA = -3,     /* CUDA runtime error, or no device              */
   GM_ERR_OVERFLOW = -4, /* scattered-superphoton queue cannot hold one batch of minimum size */
-  GM_ERR_GRID = -5      /* non-finite value in the fluid grid            */
+  GM_ERR_GRID = -5,     /* non-finite value in the fluid grid            */
+  GM_ERR_BOUND = -6     /* a cold-pass upper bound was exceeded by the exact value (gm_stats.n_bound_violations): the run's tally is void */
 };
 
 /* POD parameter block, copied at gm_create.  Field meaning: the comments below and DESIGN.md section 2 (readings G0-G33);
@@ -83,7 +84,9 @@ typedef struct gm_stats {
       n_maxstep, n_outofrange, n_steps_total, n_verlet_iters, n_verlet_capped, n_bad_scatter,
       n_analog_killed,
       n_steps_free,   /* of n_steps_total: steps taken in free flight beyond the grid (escape kernel) */
-      n_reentered;    /* superphotons that came back into the grid from free flight                  */
+      n_reentered,    /* superphotons that came back into the grid from free flight                  */
+      n_bound_violations; /* records whose exact scattering opacity / bias / Theta_e exceeded the per-cell upper bound the cold
+                             pass had decided a step with; any non-zero value makes gm_run fail (GM_ERR_BOUND) */
   double sum_w_emit, sum_w_rec, sum_w_horizon, sum_w_roulette_killed, sum_w_roulette_gain,
       sum_w_outofrange, sum_w_maxstep, sum_w_absorbed, sum_wE_emit, sum_wE_rec, sum_w_bad,
       sum_w_spawned;  /* total weight w/b given to scattered superphotons                       */

@@ -15,7 +15,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 # GPUMONTY_B200_LIB selects another build of the same library (tuning experiments: launch bounds etc.)
 LIB_PATH = os.environ.get("GPUMONTY_B200_LIB") or os.path.join(_HERE, "libgpumonty_b200.so")
 
-GM_ABI_VERSION = 2
+GM_ABI_VERSION = 3
 TABLE_LNK2, TABLE_LNF, TABLE_LNSIGH, TABLE_LNW, TABLE_NEXP, TABLE_QMAX = range(6)
 EVAL_ACCEL, EVAL_GEOM, EVAL_PLASMA, EVAL_OPAC, EVAL_PUSH, EVAL_RAD, EVAL_NB, EVAL_BOUND = range(8)
 _EVAL_SHAPES = {EVAL_ACCEL: (8, 4), EVAL_GEOM: (4, 33), EVAL_PLASMA: (4, 12), EVAL_OPAC: (8, 3),
@@ -53,7 +53,7 @@ class GmStats(C.Structure):
     _fields_ = [(n, C.c_int64) for n in (
         "n_primary", "n_spawned", "n_recorded", "n_horizon", "n_roulette_killed", "n_roulette_survived",
         "n_maxstep", "n_outofrange", "n_steps_total", "n_verlet_iters", "n_verlet_capped", "n_bad_scatter",
-        "n_analog_killed", "n_steps_free", "n_reentered")] + [(n, C.c_double) for n in (
+        "n_analog_killed", "n_steps_free", "n_reentered", "n_bound_violations")] + [(n, C.c_double) for n in (
         "sum_w_emit", "sum_w_rec", "sum_w_horizon", "sum_w_roulette_killed", "sum_w_roulette_gain",
         "sum_w_outofrange", "sum_w_maxstep", "sum_w_absorbed", "sum_wE_emit", "sum_wE_rec", "sum_w_bad",
         "sum_w_spawned")]

@@ -4,6 +4,7 @@
 #include "gm_host.h"
 #include <cmath>
 #include <cstdarg>
+#include <cstddef>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -173,6 +174,8 @@ static void fill_dev_params(gm_ctx* c) {
   P.nu_lo = p.nu_lo; P.db = std::log(p.nu_hi / p.nu_lo) / p.n_nu; P.inv_db = 1.0 / P.db;
   P.seed_lo = (uint32_t)(p.seed & 0xffffffffu); P.seed_hi = (uint32_t)(p.seed >> 32);
   P.cellB = c->d_cellB;
+  P.bound_debug_scale = 1.0;
+  if (const char* e = getenv("GPUMONTY_B200_BOUND_SCALE")) { const double v = atof(e); if (v > 0.0 && std::isfinite(v)) P.bound_debug_scale = v; }
   P.prim = c->d_prim; P.lnK2 = c->d_lnK2; P.lnF = c->d_lnF; P.lnSigH = c->d_lnSigH; P.lnw = c->d_lnw;
 }
 
@@ -428,8 +431,9 @@ static int ensure_run_buffers(gm_ctx* ctx, long long n_ids) {
   long long queue = queue_for(batch);
   // size the batch from the free device memory (at most half of it)
   const int pairs = phase_pairs_of(ctx);
-  auto bytes = [&](long long b, long long q) {
-    return (size_t)(b + 2 * q + (pairs > 0 ? 3 : 1) * (b > q ? b : q)) * sizeof(Photon);
+  const bool want_wstack = ctx->p.scattering_on && ctx->cascade_max > 0;
+  auto bytes = [&](long long b, long long q) {      // everything allocated below, the cascade's event stacks included
+    return (size_t)(b + 2 * q + (pairs > 0 ? 3 : 1) * (b > q ? b : q) + (want_wstack ? track_wstack_records(ctx->n_sm) : 0)) * sizeof(Photon);
   };
   ctx->batch_limited_by_memory = false;
   while (bytes(batch, queue) > free_b / 2 && batch > 1024) { batch >>= 1; queue = queue_for(batch); ctx->batch_limited_by_memory = true; }
@@ -440,7 +444,7 @@ static int ensure_run_buffers(gm_ctx* ctx, long long n_ids) {
   if (e == cudaSuccess) e = cudaMalloc((void**)&ctx->d_esc, (size_t)esc * sizeof(Photon));
   if (e == cudaSuccess && pairs > 0) e = cudaMalloc((void**)&ctx->d_parkA, (size_t)esc * sizeof(Photon));
   if (e == cudaSuccess && pairs > 0) e = cudaMalloc((void**)&ctx->d_parkB, (size_t)esc * sizeof(Photon));
-  if (e == cudaSuccess && ctx->p.scattering_on && ctx->cascade_max > 0)
+  if (e == cudaSuccess && want_wstack)
     e = cudaMalloc((void**)&ctx->d_wstack, (size_t)track_wstack_records(ctx->n_sm) * sizeof(Photon));
   if (e != cudaSuccess) {                        // leave no half-allocated state behind (batch_primaries stays 0)
     free_run_buffers(ctx);
@@ -488,7 +492,10 @@ static int run_batch(gm_ctx* ctx, long long first, int n, const long long* d_ids
   int mq = 0, round = 0;
   bool cascaded = false;
   for (;;) {
-    // generations 0..layers without a host round trip; afterwards only while re-entrants keep a queue non-empty
+    // generations 0..layers are enqueued back to back; the only host round trips inside this block are the schedule
+    // pilot (once per gm_prepare) and, for Kerr workloads with scattering, ONE 4-byte read-back per generation from
+    // generation 1 on that decides when the cascade pass starts (so gm_run is not asynchronous within a batch);
+    // afterwards rounds continue only while re-entrants keep a queue non-empty
     // first block: the nominal generations; afterwards one round per host check (re-entrants from free flight and
     // the descendants of stragglers that were carried into the last nominal round)
     const bool first_block = round == 0;
@@ -574,6 +581,10 @@ static int run_batch(gm_ctx* ctx, long long first, int n, const long long* d_ids
       *max_queue = qcap + 1;
       return GM_OK;
     }
+    if (h_counts[67] & 4)
+      return fail(ctx, GM_ERR_BOUND, "cold-pass bound violated: a superphoton's exact scattering opacity, bias or Theta_e exceeded the "
+                  "per-cell upper bound a bounded step was decided with (gm_stats.n_bound_violations); the tally of this run is not "
+                  "valid.  Run with gm_set_phase_passes(ctx, 0, ...) (no bounded steps) and report the grid");
     if (h_counts[67] != 0 || h_counts[64] > parkA.capacity || h_counts[65] > parkB.capacity || h_counts[2] > esc.capacity)
       return fail(ctx, GM_ERR_OVERFLOW, "internal queue overflow (flags %d; free-flight %d/%d, hand-over %d, %d/%d records)",
                   h_counts[67], h_counts[2], esc.capacity, h_counts[64], h_counts[65], parkA.capacity);
@@ -602,7 +613,7 @@ static int run_range(gm_ctx* ctx, int64_t first_id, int64_t n_ids, Tally tally, 
     CK(cudaMemcpyAsync(ctx->d_stats_snap, stats, sizeof(DevStats), cudaMemcpyDeviceToDevice, st));
     int mq = 0;
     r = run_batch(ctx, first_id + done, (int)nthis, nullptr, notrace, false, tally, stats, st, &mq);
-    if (r != GM_OK) return r;
+    if (r != GM_OK) { ctx->cascade_skip = false; ctx->cascade_overflowed = false; return r; }
     if (mq > ctx->queue_records) {
       CK(cudaMemcpyAsync(tally.A, ctx->tally_snap.A, (size_t)nb * 4 * sizeof(double), cudaMemcpyDeviceToDevice, st));
       CK(cudaMemcpyAsync(stats, ctx->d_stats_snap, sizeof(DevStats), cudaMemcpyDeviceToDevice, st));
@@ -657,11 +668,24 @@ static int tune_bias(gm_ctx* ctx, cudaStream_t st) {
   for (int g = 0; g < 64; g++) { best_fac[g] = 1.0; best_err[g] = 1e300; low_base[g] = 1.0; last_spawned[g] = -1; low_fail[g] = in_low[g] = frozen[g] = 0; }
   int rc = GM_OK;
   DevStats* h = new DevStats;
+  double prev_fac[64];                                     // factors of the last pilot pass that ran to its end
+  for (int g = 0; g < 64; g++) prev_fac[g] = ctx->P.bias_fac[g];
   for (int iter = 0; iter < 2 * G + 8 && rc == GM_OK; iter++) {
-    cudaMemsetAsync(d_tl, 0, (size_t)nb * 4 * sizeof(double), st);
-    cudaMemsetAsync(d_st, 0, sizeof(DevStats), st);
+    if (cudaMemsetAsync(d_tl, 0, (size_t)nb * 4 * sizeof(double), st) != cudaSuccess ||
+        cudaMemsetAsync(d_st, 0, sizeof(DevStats), st) != cudaSuccess) {
+      rc = fail(ctx, GM_ERR_CUDA, "tune_bias: clearing the scratch tally failed"); break;
+    }
     rc = run_range(ctx, 0, n_pilot, scratch, d_st, st);
+    if (rc == GM_ERR_OVERFLOW && iter > 0) {
+      // the last update (a x16 or x4 climb) spawns more than the scattered queue holds even for the smallest batch:
+      // the queue capacity caps the climb -- take the step back, freeze those generations, go on with the others
+      bool any = false;
+      for (int g = 0; g < G; g++)
+        if (ctx->P.bias_fac[g] != prev_fac[g]) { ctx->P.bias_fac[g] = prev_fac[g]; frozen[g] = 1; any = true; }
+      if (any) { rc = GM_OK; continue; }
+    }
     if (rc != GM_OK) break;
+    for (int g = 0; g < 64; g++) prev_fac[g] = ctx->P.bias_fac[g];
     if (cudaMemcpyAsync(h, d_st, sizeof(DevStats), cudaMemcpyDeviceToHost, st) != cudaSuccess || cudaStreamSynchronize(st) != cudaSuccess) {
       rc = fail(ctx, GM_ERR_CUDA, "tune_bias: read-back failed"); break;
     }
@@ -703,6 +727,10 @@ static int tune_bias(gm_ctx* ctx, cudaStream_t st) {
   }
   delete h;
   cudaFree(d_tl); cudaFree(d_st);
+  if (rc != GM_OK) {                                       // no half-tuned table behind a failed gm_prepare
+    for (int g = 0; g < 64; g++) ctx->P.bias_fac[g] = 1.0;
+    ctx->prepared = false;
+  }
   return rc;
 }
 
@@ -764,7 +792,8 @@ int gm_get_stats(gm_ctx* ctx, gm_stats* out) {
   CK(cudaDeviceSynchronize());
   CK(cudaMemcpy(&h, ctx->d_stats, sizeof(h), cudaMemcpyDeviceToHost));
   int64_t* ni = &out->n_primary;
-  for (int i = 0; i < 15; i++) ni[i] = (int64_t)h.n[i];
+  static_assert(offsetof(gm_stats, n_bound_violations) == 15 * sizeof(int64_t) && offsetof(gm_stats, sum_w_emit) == 16 * sizeof(int64_t), "gm_stats layout");
+  for (int i = 0; i < 16; i++) ni[i] = (int64_t)h.n[i];
   double* sd = &out->sum_w_emit;
   for (int i = 0; i < 12; i++) sd[i] = h.s[i];
   return GM_OK;

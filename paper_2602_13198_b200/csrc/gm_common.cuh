@@ -70,6 +70,8 @@ struct DevParams {
   // per interpolation cell (indexed like its lowest corner zone): {S, Theta_B}, upper bounds of the scattering
   // opacity per unit k^t and of Theta_e anywhere in the cell (cell_bound_kernel; the tracker's cold pass)
   const double2* __restrict__ cellB;
+  double bound_debug_scale;                           // 1; GPUMONTY_B200_BOUND_SCALE (read at gm_create) multiplies S: lets a test
+                                                      // shrink the bound on purpose and watch the run-time guard fire
 };
 
 // ---- superphoton record (160 B, 16-B aligned) -------------------------------------------------
@@ -83,12 +85,13 @@ static_assert(sizeof(Photon) == 160, "Photon record must be 160 bytes");
 
 // per-run device accumulators
 struct DevStats {
-  unsigned long long n[15];
+  unsigned long long n[16];
   double s[12];
   unsigned long long gen[64];                         // scattered superphotons spawned by generation n_sc (G32)
 };
 enum { SN_PRIMARY = 0, SN_SPAWNED, SN_RECORDED, SN_HORIZON, SN_ROUL_KILLED, SN_ROUL_SURV, SN_MAXSTEP,
-       SN_OUTOFRANGE, SN_STEPS, SN_VITERS, SN_VCAPPED, SN_BADSCAT, SN_ANALOG, SN_STEPS_FREE, SN_REENTER };
+       SN_OUTOFRANGE, SN_STEPS, SN_VITERS, SN_VCAPPED, SN_BADSCAT, SN_ANALOG, SN_STEPS_FREE, SN_REENTER,
+       SN_BOUND_VIOL /* FLAG_BOUND records whose exact opacities exceeded the bounds they carried (must stay 0) */ };
 enum { SS_EMIT = 0, SS_REC, SS_HORIZON, SS_ROUL_KILLED, SS_ROUL_GAIN, SS_OUTOFRANGE, SS_MAXSTEP,
        SS_ABSORBED, SS_WE_EMIT, SS_WE_REC, SS_BAD, SS_SPAWNED };
 

@@ -393,7 +393,7 @@ __global__ void cell_bound_kernel(const DevParams P, double2* __restrict__ cellB
   const double gamB = sqrt(1.0 + 100.0 * q_max);
   // (x 1.01: the decomposition k = E_n (n + n^) assumes a null k; the integrated k.k drifts from 0 by a small multiple of
   // verlet_tol, which lets the spatial part exceed E_n by that much)
-  double S = (gamB + sqrt(100.0 * q_max)) * (rho_max * P.Ne_unit) * C_SIGT * C_MEC2_H * 1.01;
+  double S = (gamB + sqrt(100.0 * q_max)) * (rho_max * P.Ne_unit) * C_SIGT * C_MEC2_H * 1.01 * P.bound_debug_scale;
   if (!ok || !isfinite(S) || !isfinite(thB)) { S = INFINITY; thB = INFINITY; }
   cellB[z] = make_double2(S, thB);
 }

@@ -659,6 +659,11 @@ track_kernel(const __grid_constant__ DevParams P, const Photon* __restrict__ in,
     }
 
     if (PHASE != PHASE_COLD && mode == 3) {                // zero-length step of a FLAG_BOUND record: its exact opacities
+      // run-time guard of the cold pass: the record still carries the bounds its last bounded step was decided with.
+      // The factors in cell_bound_kernel are a heuristic, not a proof: an exact value above its bound (or absorbing
+      // plasma where the bound said none) means a decision of the cold pass may have been wrong -> counted, and
+      // flagged to the host, which fails the run (gm_run: GM_ERR_BOUND)
+      if ((ns1 > L.nua_s) | (b1 > L.bias) | hot) { atomicAdd(&stats->n[SN_BOUND_VIOL], 1ull); atomicOr(overflow, 4); }
       L.nua_s = ns1; L.bias = b1; L.flags &= ~FLAG_BOUND;
       mode = 0;
       continue;

@@ -46,7 +46,7 @@ def calibrated() -> dict:
 
 def default_params() -> dict:
     return dict(
-        abi_version=2, seed=1, Ns_target=1e5,
+        abi_version=3, seed=1, Ns_target=1e5,
         metric_kind=0, a_spin=0.0, hslope=1.0,
         startx=[0.0, 0.0, 0.0, 0.0], dx=[1.0, 1.0, 1.0, 2.0 * math.pi],
         n1=1, n2=1, n3=1,

@@ -33,7 +33,7 @@ def _report(line):
             f.write(line + "\n")
 
 
-def _criterion(cfg, A_o, Q_o, n_o, A_g, n_g, min_count=1000):
+def _criterion(cfg, A_o, Q_o, n_o, A_g, n_g, min_count=1000, min_bins=None):
     """Every bin with >= min_count superphotons (oracle count): |A_g/A_o - 1| < 1 % and |A_g - A_o| < 3 sqrt(Q_o).
     nu L_nu and its sigma are A and sqrt(Q) times one common factor per theta bin, so the ratio and the sigma
     distance are those of the spectra."""
@@ -44,7 +44,7 @@ def _criterion(cfg, A_o, Q_o, n_o, A_g, n_g, min_count=1000):
     dn = np.abs(n_g.astype(np.int64) - n_o.astype(np.int64))
     _report(f"| cfg{cfg} | {nsel} | {rel.max():.3e} | {nsig.max():.3e} | {int((dn > 0).sum())} | {int(dn.max())} | "
             f"{int(n_o.sum())} | {int(n_g.sum())} |")
-    assert nsel >= MIN_BINS[cfg], (cfg, nsel)
+    assert nsel >= (MIN_BINS[cfg] if min_bins is None else min_bins), (cfg, nsel)
     assert np.all(rel < 0.01), rel.max()
     assert np.all(nsig < 3.0), nsig.max()
     # counts per bin equal up to forked histories: a fork moves one superphoton (and its descendants) elsewhere
@@ -95,7 +95,8 @@ def test_config0_full_size_spectrum(gm):
     assert np.array_equal(o.zone_counts(), g.zone_counts())
     A_o, Q_o, W_o, n_o = o.tally()
     A_g, Q_g, W_g, n_g = g.tally()
-    _criterion(0, A_o, Q_o, n_o, A_g, n_g, min_count=900)
+    _criterion(0, A_o, Q_o, n_o, A_g, n_g, min_count=1000, min_bins=12)   # the stated bar: 16 bins reach 1000 at this N_s
+    _criterion(0, A_o, Q_o, n_o, A_g, n_g, min_count=900)                  # and the whole populated band (33 bins)
 
 
 @pytest.mark.parametrize("cfg", [1, 2, 3, 4])
@@ -119,6 +120,7 @@ def test_full_size_spectrum_against_the_stored_oracle_tally(gm, cfg):
     so = dict(zip([str(k) for k in gold["stats_keys"]], gold["stats_vals"]))
     sg = g.stats()
     assert sg["n_primary"] == so["n_primary"]
+    assert sg["n_bound_violations"] == 0          # run-time guard of the cold pass's per-cell bounds (gm_run fails otherwise)
     for k in ("n_spawned", "n_recorded", "n_steps_total", "n_horizon", "n_roulette_killed"):
         assert abs(sg[k] - so[k]) <= max(3, 2e-4 * so[k]), (k, sg[k], so[k])
     for k in ("sum_w_emit", "sum_wE_emit"):

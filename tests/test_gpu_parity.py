@@ -3,11 +3,13 @@ same seeded inputs and the same Philox streams (SURVEY.md 8(c) "History divergen
 
 Tolerances (DESIGN.md section 3 "Tolerances of the GPU parity tests"):
   * integer / index work (Philox words, zone counts, prefix sum, bins, step counts): bit-exact;
-  * device functions evaluated at the same point: 1e-11 relative (libdevice vs glibc last-ulp differences,
-    closed-form vs generic-inverse metric algebra), tables 1e-9 (K2, F) / 3e-7 (sigma_h: the oracle's own
-    quadrature tolerance is 1e-8);
-  * per-history final state: |dw/w|, |dE/E| < 1e-7 for histories that did not fork; forked histories
-    (a uniform within rounding of a threshold) must stay below 1e-3 of the sample;
+  * device functions evaluated at the same point: 1e-10 relative on geometry, wavevectors, weights and opacities
+    (libdevice vs glibc last-ulp differences, closed-form vs generic-inverse metric algebra; the assertions below carry
+    their own figure where it differs), tables 1e-12 (K2, F) / 3e-7 (sigma_h: the oracle's own quadrature tolerance
+    is 1e-8);
+  * per-history final state: |dw/w|, |dE/E| < 1e-7 for histories that did not fork; final position within
+    1e-7 max(1, nstep/300); forked histories (a uniform within rounding of a threshold) must stay below 2e-4 of the
+    sample (measured: 0 in 68,000, profiles/r02_parity.md);
   * spectra: north_star's bar -- every bin holding >= 1000 superphotons within 1 % and within 3 sigma; at full
     size in tests/test_gpu_full_size.py, here on the bins above a stated lower count (their number asserted).
 """
@@ -310,10 +312,39 @@ def test_scan_ragged_tail_and_empty_zones(gm):
     assert (cg == 0).sum() > 100 and cg.sum() == g.n_primaries
 
 
+def test_run_time_guard_of_the_cold_pass_bounds(gm, monkeypatch):
+    """The per-cell bounds of the cold pass rest on heuristic factors, so every record that comes
+    back from a bounded step is checked in the hot pass against the exact values: exact nu alpha_s <= bound, exact bias
+    <= bound, no absorbing plasma where the bound said none.  With the real bounds the counter stays 0; with S shrunk on
+    purpose (GPUMONTY_B200_BOUND_SCALE, read at gm_create) the counter rises and gm_run refuses to return a tally."""
+    p, prim = wl.config2(Ns=3e5)
+    g = gm.GPUMonty(p)
+    g.set_phase_passes(3, 4)                                 # bounded cold passes forced (the batch is below the automatic size)
+    g.set_grid(prim); g.prepare(); g.run()
+    s0 = g.stats()
+    assert s0["n_bound_violations"] == 0 and s0["n_spawned"] > 0
+    monkeypatch.setenv("GPUMONTY_B200_BOUND_SCALE", "0.02")
+    h = gm.GPUMonty(p)
+    monkeypatch.delenv("GPUMONTY_B200_BOUND_SCALE")
+    h.set_phase_passes(3, 4)
+    h.set_grid(prim); h.prepare()
+    with pytest.raises(gm.GmError) as e:
+        h.run()
+    assert e.value.code == -6 and "bound" in str(e.value)      # GM_ERR_BOUND
+    assert h.stats()["n_bound_violations"] > 0
+    # without bounded steps the same context gives the reference run again: the guard protects, it does not alter
+    h.set_phase_passes(0, 4)
+    h.reset_tally(); h.prepare(); h.run()
+    s1 = h.stats()
+    assert s1["n_bound_violations"] == 0
+    for k in ("n_primary", "n_spawned", "n_recorded", "n_steps_total"):
+        assert s1[k] == s0[k], k
+
+
 # ---------------------------------------------------------------------------------------------------
 # S6-S12: histories and spectra
 # ---------------------------------------------------------------------------------------------------
-def _compare_traces(o, g, ids, fork_budget, label=None, x_tol=1e-7):
+def _compare_traces(o, g, ids, fork_budget, label=None):
     """Same-stream histories one by one.  A history "forks" when a uniform falls within rounding of a threshold
     (or libdevice and glibc differ in the last ulp of a transcendental): every integer of its final state is
     compared, the forks are counted, printed and (on the GPU box) appended to gpurun_out/fork_rates.md; the budget
@@ -336,11 +367,20 @@ def _compare_traces(o, g, ids, fork_budget, label=None, x_tol=1e-7):
     assert np.max(_relerr(tg["w"][ok], to["w"][ok])) < 1e-7
     rec = ok[to["fate"][ok] == 1]
     assert np.max(_relerr(tg["E_inf"][rec], to["E_inf"][rec])) < 1e-7
+    # final position: 1e-7, growing with the length of the history beyond 300 steps (rounding-order differences of 1e-16
+    # per step are amplified along a geodesic; DESIGN.md section 3 and profiles/r03_parity.md show the same growth on the
+    # oracle alone under a 1-ulp perturbation).  Short histories stay held to 1e-7.
     dx = np.max(np.abs(tg["x"][ok] - to["x"][ok]), axis=1)
-    if x_tol != 1e-7:
-        print("largest final-position difference %.2e (history of %d steps); %d of %d above 1e-7"
-              % (dx.max(), tg["nstep"][ok][np.argmax(dx)], np.count_nonzero(dx >= 1e-7), len(ok)))
-    assert dx.max() < x_tol
+    x_tol = 1e-7 * np.maximum(1.0, to["nstep"][ok] / 300.0)
+    worst = int(np.argmax(dx / x_tol))
+    wline = "| %s | %d | %.2e | %d | %d | %d |" % (label or os.environ.get("PYTEST_CURRENT_TEST", "?").split("::")[-1].split(" ")[0],
+                                                 len(ok), dx[worst], int(np.asarray(ids)[ok][worst]), to["nstep"][ok][worst],
+                                                 np.count_nonzero(dx >= 1e-7))
+    print("largest final-position difference (x / id / steps / above 1e-7) " + wline)
+    if os.path.isdir("gpurun_out"):
+        with open(os.path.join("gpurun_out", "position_differences.md"), "a") as f:
+            f.write(wline + "\n")
+    assert np.all(dx < x_tol), (dx[worst], to["nstep"][ok][worst])
     # family sums: only compare where the spawn counts agree (a fork inside a child changes them)
     assert len(fsame) >= (1 - 10 * fork_budget) * len(ok) - 1
     assert np.max(_relerr(tg["fam_wE"][fsame], fam_wE[fsame], floor=1e-300)) < 1e-6
@@ -686,10 +726,7 @@ def _full_size_checks(gm, p, prim, n_sample, seed):
            sg["sum_w_outofrange"] + sg["sum_w_maxstep"] + sg["sum_w_absorbed"] + sg["sum_w_bad"])
     assert out == pytest.approx(sg["sum_w_emit"], rel=1e-9)
     ids = np.sort(np.random.default_rng(seed).choice(g.n_primaries, n_sample, replace=False))
-    # (20,000 histories: rounding-order differences of 1e-16 per step are amplified along the longest ones -- thousands of
-    # small steps next to the polar axis -- to just above the 1e-7 that the smaller samples never reach; every integer of
-    # those histories is still equal.  DESIGN.md section 3.)
-    _compare_traces(o, g, ids, fork_budget=2e-4, x_tol=1e-6)
+    _compare_traces(o, g, ids, fork_budget=2e-4)
     return sg
 
 
@@ -704,6 +741,23 @@ def test_full_size_config1(gm):
     """BASELINE configs[1] at N_s = 1e6."""
     p, prim = wl.config1()
     _full_size_checks(gm, p, prim, 20000, 22)
+
+
+def test_full_size_config3(gm):
+    """BASELINE configs[3] as bench.py times it: the full 192 x 128 x 128 grid at N_s = 1e7 with the AUTOMATIC schedule
+    (hot / bounded-cold passes chosen by the pilot): zone counts of the 3,145,728 zones bit-exact against the oracle's
+    at this N_s (w_min and the counts scale with it), sampled histories one by one."""
+    p, prim = wl.config3()
+    assert p["Ns_target"] == 1e7 and (p["n1"], p["n2"], p["n3"]) == (192, 128, 128)
+    sg = _full_size_checks(gm, p, prim, 5000, 23)
+    assert sg["n_bound_violations"] == 0
+
+
+def test_full_size_config4(gm):
+    """BASELINE configs[4] at the N_s bench.py's other_configs line times (1e7), automatic schedule."""
+    p, prim = wl.config4(Ns=1e7)
+    sg = _full_size_checks(gm, p, prim, 5000, 24)
+    assert sg["n_bound_violations"] == 0
 
 
 def test_batching_and_queue_overflow_recovery(gm):
