@@ -349,3 +349,89 @@ def test_oracle_tally_statistics():
         assert np.all(A[m] ** 2 <= Q[m] * n[m] * (1 + 1e-12))         # Cauchy-Schwarz: n_eff <= n
         med[c] = float(np.median(A[m] ** 2 / Q[m] / n[m]))
     assert med[1] > 0.1 and max(med[2], med[3], med[4]) < 0.01, med
+
+
+# ---------------------------------------------------------------------------------------------------
+# (e) gather at a point beyond the polar axis (reading G33)
+# ---------------------------------------------------------------------------------------------------
+def _tilted_field_grid(n2, n3, alpha):
+    """Static uniform sphere in flat space on a 3-D grid, with two things that are NOT axisymmetric: the field
+    B = B0 (sin(alpha) e_x + cos(alpha) e_z), a constant Cartesian vector written in spherical components at the zone
+    centres, and the density rho = n0 (1 + 0.3 x / r)."""
+    n1 = 8
+    p, prim = wl.sphere(1e13, 10.0, 1.0, R, n1, n2, 1e3, 1, False)
+    p.update(n3=n3, dx=[1.0, p["dx"][1], p["dx"][2], 2 * math.pi / n3])
+    prim = np.repeat(prim, n3, axis=2)
+    x1 = p["startx"][1] + (np.arange(n1) + 0.5) * p["dx"][1]
+    x2 = (np.arange(n2) + 0.5) * p["dx"][2]
+    x3 = (np.arange(n3) + 0.5) * p["dx"][3]
+    r, th, ph = np.meshgrid(np.exp(x1), math.pi * x2, x3, indexing="ij")
+    B0 = math.hypot(prim[0, 0, 0, 5] * r[0, 0, 0], prim[0, 0, 0, 6] * r[0, 0, 0] * math.pi)
+    sa, ca = math.sin(alpha), math.cos(alpha)
+    Br = sa * np.sin(th) * np.cos(ph) + ca * np.cos(th)
+    Bt = sa * np.cos(th) * np.cos(ph) - ca * np.sin(th)
+    Bp = -sa * np.sin(ph)
+    prim[..., 5] = B0 * Br / r
+    prim[..., 6] = B0 * Bt / (r * math.pi)
+    prim[..., 7] = B0 * Bp / (r * np.sin(th))
+    prim[..., 0] *= 1.0 + 0.3 * np.sin(th) * np.cos(ph)
+    return p, np.ascontiguousarray(prim), B0, x1
+
+
+def _cartesian(x, v):
+    """Cartesian components of the spatial part of a vector given in (x1 = ln r, x2 = theta/pi, x3 = phi) components at
+    x; the same analytic formulas serve for x2 < 0 (theta continued through the pole)."""
+    r, th, ph = math.exp(x[1]), math.pi * x[2], x[3]
+    st, ct, sp, cp = math.sin(th), math.cos(th), math.sin(ph), math.cos(ph)
+    rh = np.array([st * cp, st * sp, ct]); thh = np.array([ct * cp, ct * sp, -st]); phh = np.array([-sp, cp, 0.0])
+    return (r * v[1]) * rh + (r * math.pi * v[2]) * thh + (r * st * v[3]) * phh
+
+
+@pytest.mark.parametrize("pole", [0.0, 1.0])
+def test_gather_beyond_the_polar_axis_is_the_continuous_continuation_of_the_clamped_half_zone(pole):
+    """G33.  A push can end at x2 < 0 or x2 > 1; the plasma state is needed there once before the photon is reflected
+    (G14).  The oracle mirrors x2 and reads the same azimuth with unchanged components.  The first-order part of a step
+    cannot reach the axis (|k^2| dl <= step_eps * distance, G16): only the curvature term carries a point across, by a
+    small fraction of a zone, i.e. deep inside the mirror image of the half zone next to the axis, where the
+    interpolation (G4) is clamped to the outermost zone centre.  So this reading is: the clamped half-zone state
+    continued as a constant through the pole.  Pinned here on a field and a density that are NOT axisymmetric:
+      (1) continuous: the state at -eps equals the state at +eps (to rounding), for every quantity returned;
+      (2) no worse than the clamp itself: against the exact smooth fields at the physical point (density; Cartesian
+          direction of b) the error at a distance d <= 0.1 zone beyond the axis stays within 1.7x the error at the same
+          distance inside, and the density error is first order in dtheta (halves from n2 = 16 to 32) on both sides;
+      (3) the mirror is about the axis: 1.5 zones beyond it the state is that of the point 1.5 zones inside.
+    The alternative reading (azimuth + pi, x2-components negated) is exact for a smooth field, but applied to the
+    CLAMPED half zone it jumps at the pole (by 2 sin(dtheta/2) in the direction of b for an axisymmetric field);
+    DESIGN.md G33 states both."""
+    errs = {}
+    for n2 in (16, 32):
+        p, prim, B0, x1 = _tilted_field_grid(n2, 16, 0.7)
+        o = Oracle(p, prim)
+        bdir = np.array([math.sin(0.7), 0.0, math.cos(0.7)])
+        sgn = -1.0 if pole == 0.0 else 1.0                       # direction "beyond the axis"
+        w = {"in": [0.0, 0.0], "out": [0.0, 0.0]}                # worst (density error, direction error)
+        for phi in (0.3, 2.0, 4.4):
+            for d in (1e-9, 0.02 * p["dx"][2], 0.1 * p["dx"][2]):
+                xin = np.array([0.0, x1[3], pole - sgn * d, phi])
+                xout = np.array([0.0, x1[3], pole + sgn * d, phi])
+                Sin, Sout = o.plasma_at(xin), o.plasma_at(xout)
+                if d == 1e-9:                                    # (1)
+                    for k in ("ne", "thetae", "B"):
+                        assert Sout[k] == pytest.approx(Sin[k], rel=1e-12)
+                    assert np.allclose(Sout["bcon"], Sin["bcon"], rtol=0, atol=1e-7 * np.abs(Sin["bcon"]).max())
+                    assert np.allclose(Sout["ucon"], Sin["ucon"], rtol=0, atol=1e-12)
+                for S, xx, which in ((Sin, xin, "in"), (Sout, xout, "out")):
+                    th, ph = math.pi * xx[2], xx[3]
+                    ne_exact = 1e13 * (1.0 + 0.3 * math.sin(th) * math.cos(ph))     # analytic in theta through the pole
+                    bc = _cartesian(xx, S["bcon"])
+                    w[which][0] = max(w[which][0], abs(S["ne"] / ne_exact - 1.0))
+                    w[which][1] = max(w[which][1], float(np.linalg.norm(bc / np.linalg.norm(bc) - bdir)))
+        errs[n2] = w
+        assert w["out"][0] < 1.7 * w["in"][0] and w["out"][1] < 1.7 * w["in"][1], errs      # (2)
+        assert w["in"][0] > 1e-3                                 # (the comparison is not between two zeros)
+        xfar = np.array([0.0, x1[3], pole + sgn * 1.5 * p["dx"][2], 0.3])                    # (3)
+        xmir = np.array([0.0, x1[3], pole - sgn * 1.5 * p["dx"][2], 0.3])
+        assert o.plasma_at(xfar)["ne"] == pytest.approx(o.plasma_at(xmir)["ne"], rel=1e-12)
+        assert o.plasma_at(xfar)["ne"] != pytest.approx(o.plasma_at(xin)["ne"], rel=1e-4)
+    for side in ("in", "out"):
+        assert errs[32][side][0] < 0.62 * errs[16][side][0], errs                          # first order in dtheta
