@@ -11,7 +11,8 @@ The five BASELINE.json configs leave three numbers per config open (SURVEY.md 8(
            it (the paper's own floor, 1e28, is likewise ~1e-17 of its typical weights).
   M_unit   mass unit of the torus configs.  BASELINE.json asks for ~2.5 Jy at 230 GHz; for this
            synthetic torus (R_high = 40, beta = 100 => Theta_e ~ 0.4) the 230 GHz flux of the
-           oracle peaks near 0.5 Jy at M_unit ~ 1e23 (Thomson depth ~2) and collapses beyond it, so
+           oracle peaks at 0.54 Jy at M_unit = 1e23 (equatorial Thomson depth 1.15) and collapses beyond it
+           (--munit-scan below writes that curve), so
            the target is unreachable; M_unit = 5e19 is fixed instead, which gives the Thomson depths
            BASELINE.json states for config 4 (tau_T ~ 1 after the x1e3 density scaling).  The
            measured 230 GHz flux is stored for the record.
@@ -19,6 +20,11 @@ The five BASELINE.json configs leave three numbers per config open (SURVEY.md 8(
            ("7-10x"); config 1 uses 0.25/tau_T; config 4 is analog (b = 1).
 
 Run:  python oracle/calibrate.py        (about two minutes on 8 cores; deterministic)
+      python oracle/calibrate.py --munit-scan
+          adds the key "cfg2_munit_scan" to the same file and changes nothing else in it: the 230 GHz flux of the
+          config-2 torus (oracle, N_s = 1e5, no scattering, 45-75 degree bins) and its equatorial Thomson depth for
+          M_unit = 1e19 .. 1e25 in half decades -- the curve behind the sentence above that 2.5 Jy is out of reach
+          (BASELINE.md section 4 quotes its maximum).
 Nothing here touches the CUDA path.
 """
 import json
@@ -81,7 +87,38 @@ def flux230(p, prim):
     return float(spec[3:5, j - 1:j + 2].mean() / (4 * math.pi * D * D * nub[j]) / 1e-23)
 
 
+def thomson_depth_equator(p, prim):
+    """sigma_T * integral of n_e dr along the equatorial ray of the grid (the two rows next to x2 = 1/2 averaged)."""
+    RHO = p["M_unit"] / p["L_unit"] ** 3
+    ne = prim[:, :, 0, 0] * RHO / (wl.MP + wl.ME)
+    j = p["n2"] // 2
+    r = np.exp(p["startx"][1] + (np.arange(p["n1"]) + 0.5) * p["dx"][1]) * p["L_unit"]
+    return float(wl.SIGMA_T * np.sum(0.5 * (ne[:, j - 1] + ne[:, j]) * r * p["dx"][1]))
+
+
+def munit_scan():
+    p, prim = wl.torus(256, 256, 1, Ns=1e7, seed=1)
+    rows = []
+    for e2 in range(38, 51):                    # M_unit = 10^(e2/2): 1e19, 3.2e19, ..., 1e25
+        p["M_unit"] = 10.0 ** (0.5 * e2)
+        rows.append({"M_unit": p["M_unit"], "F230_Jy_45_75deg": flux230(p, prim), "tau_T_equator": thomson_depth_equator(p, prim)})
+        print(rows[-1], flush=True)
+    best = max(rows, key=lambda r: r["F230_Jy_45_75deg"])
+    cal = json.load(open(OUT))
+    cal["cfg2_munit_scan"] = {"rows": rows, "max_F230_Jy": best["F230_Jy_45_75deg"], "M_unit_at_max": best["M_unit"],
+                              "recipe": "oracle only, config-2 torus 256x256, N_s = 1e5, scattering off, nu in [1e10, 1e13] Hz, "
+                                        "flux = mean nu L_nu of theta bins 3-4 and the three frequency bins around 230 GHz / "
+                                        "(4 pi D^2 nu), D = 8.1 kpc"}
+    with open(OUT, "w") as f:
+        json.dump(cal, f, indent=1)
+        f.write("\n")
+    print("maximum %.3g Jy at M_unit = %.3g" % (best["F230_Jy_45_75deg"], best["M_unit"]))
+
+
 def main():
+    if "--munit-scan" in sys.argv:
+        munit_scan()
+        return
     cal = {}
     p, prim = wl.sphere(1e13, 10.0, 1.0, 1e3, 32, 16, 1e5, 1, False)
     cal["cfg0"] = {"w_min_per_Ns1": wmin_per_ns(p, prim)}
