@@ -378,7 +378,7 @@ def _tilted_field_grid(n2, n3, alpha):
     return p, np.ascontiguousarray(prim), B0, x1
 
 
-def _cartesian(x, v):
+def _spatial_cartesian(x, v):
     """Cartesian components of the spatial part of a vector given in (x1 = ln r, x2 = theta/pi, x3 = phi) components at
     x; the same analytic formulas serve for x2 < 0 (theta continued through the pole)."""
     r, th, ph = math.exp(x[1]), math.pi * x[2], x[3]
@@ -423,7 +423,7 @@ def test_gather_beyond_the_polar_axis_is_the_continuous_continuation_of_the_clam
                 for S, xx, which in ((Sin, xin, "in"), (Sout, xout, "out")):
                     th, ph = math.pi * xx[2], xx[3]
                     ne_exact = 1e13 * (1.0 + 0.3 * math.sin(th) * math.cos(ph))     # analytic in theta through the pole
-                    bc = _cartesian(xx, S["bcon"])
+                    bc = _spatial_cartesian(xx, S["bcon"])
                     w[which][0] = max(w[which][0], abs(S["ne"] / ne_exact - 1.0))
                     w[which][1] = max(w[which][1], float(np.linalg.norm(bc / np.linalg.norm(bc) - bdir)))
         errs[n2] = w
